@@ -1,0 +1,119 @@
+/*
+ * pf.h -- C ABI of libpf: the B200 (sm_100a) phase-field stepper.
+ *
+ * The library advances the coupled Cahn-Hilliard (conserved c) + Allen-Cahn (eta_1..eta_p) model of
+ * arXiv 2306.04322 (Boccardo, Tong, Leen, Tourret, Segurado) on a periodic 2D/3D grid:
+ *
+ *   free energy          F = int f_chem + kappa_c/2 |grad c|^2 + sum_i kappa_eta/2 |grad eta_i|^2   Eq. 1
+ *   f_chem               f^alpha (1-h) + f^beta h + w g
+ *   Cahn-Hilliard        dc/dt     = div( M grad( df/dc - kappa_c lap c ) )                         Eq. 2
+ *   Allen-Cahn           deta_i/dt = -L ( df/deta_i - kappa_eta lap eta_i )                         Eq. 3
+ *
+ * with either the semi-implicit Fourier-spectral step (Eqs. 12-15; Algorithm 1,
+ * PAPER.md:159-193) or the explicit forward-Euler 5/7-point finite-difference step.
+ * Every step of both paths runs in hand-written CUDA kernels; there is no CPU fallback: when no
+ * CUDA device is usable pf_create returns PF_ECUDA.
+ *
+ * Conventions
+ *   - fields are C-contiguous [nz][ny][nx], x fastest, index (z*ny + y)*nx + x; eta is
+ *     [n_eta][nz][ny][nx]; the element type is float (PF_F32) or double (PF_F64) as given in
+ *     pf_params.precision; host and device buffers have the same layout;
+ *   - `where` says what kind of pointer the caller passes: PF_HOST (pageable or pinned host memory)
+ *     or PF_DEVICE (device memory of the context's device). The caller owns its buffers; the library
+ *     copies and never keeps a caller pointer after the call returns;
+ *   - all work is queued on pf_params.stream (a cudaStream_t passed as void*; borrowed, never destroyed;
+ *     NULL = a private blocking stream of the context, which orders with the legacy default stream). pf_step_* and device-side set/get are asynchronous;
+ *     pf_get_fields(PF_HOST), pf_set_fields(PF_HOST) and pf_free_energy synchronise that stream;
+ *   - every call returns PF_OK (0) or a negative code; nothing throws or aborts. After PF_ECUDA
+ *     pf_last_cuda_error gives the CUDA error string.
+ */
+#ifndef PF_H
+#define PF_H
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct pf_ctx pf_ctx;     /* opaque; owns every device buffer, table and CUDA graph */
+
+enum { PF_F32 = 0, PF_F64 = 1 };
+enum { PF_HOST = 0, PF_DEVICE = 1 };
+enum { PF_OK = 0, PF_EINVAL = -1, PF_ENOMEM = -2, PF_ECUDA = -3, PF_ESTATE = -4, PF_EUNSUPPORTED = -5 };
+
+typedef struct {
+    int    ndim;            /* 2 or 3                                                                         */
+    int    n[3];            /* nx (fastest), ny, nz (= 1 when ndim == 2); powers of two, 16 .. 2048            */
+    int    n_eta;           /* p, number of Allen-Cahn order parameters, 0 .. 8 (paper: 4)        */
+    double dx[3];           /* grid spacing per axis; domain length l_d = n_d * dx_d            */
+    double dt;              /* time step                                                                       */
+    double M, L;            /* mobility, kinetic coefficient (Eqs. 2-3; paper: 5, 5)                           */
+    double kappa_c, kappa_eta;                 /* gradient-energy coefficients (Eq. 1; paper: 3, 3)            */
+    double rho2, c_alpha, c_beta, w, alpha;    /* f_chem parameters (paper: 2, .3, .7, 1, 5)   */
+    int    precision;       /* PF_F32 | PF_F64: storage and arithmetic type of every kernel                    */
+    int    k2_kind;         /* squared frequencies used by the spectral step:
+                               0 = Eq. 16/19 (Fourier spectral), 1 = Eq. 17/20 (FS-FD O(dl^2)),
+                               2 = Eq. 18/21 (FS-FD O(dl^4))                   */
+    void  *stream;          /* cudaStream_t the context runs on (NULL = private blocking stream); borrowed     */
+} pf_params;
+
+/* Creates a context on the CURRENT CUDA device: validates p, allocates all device buffers, builds
+ * the twiddle and frequency tables. *out is set only on PF_OK.
+ * PF_EINVAL: null pointers, ndim not 2/3, dt <= 0, dx <= 0, n_eta out of range, bad enum values;
+ * PF_EUNSUPPORTED: a grid size that is not a power of two in 16..2048 (nz must be 1 in 2D);
+ * PF_ENOMEM: device allocation failed; PF_ECUDA: no usable device / a CUDA call failed. */
+int pf_create(const pf_params *p, pf_ctx **out);
+
+/* Copies the fields into the context (c: [nz][ny][nx]; eta: [n_eta][nz][ny][nx], may be NULL iff
+ * n_eta == 0). Invalidates the cached spectral state. */
+int pf_set_fields(pf_ctx *ctx, const void *c, const void *eta, int where);
+
+/* nsteps semi-implicit Fourier-spectral steps (Algorithm 1):
+ *   g = df_chem/dc, h_i = df_chem/deta_i in real space
+ *   c^   <- ( c^   - dt M |xi|^2 g^   ) / ( 1 + dt M kappa_c |xi|^4 )            (Eqs. 12, 14)
+ *   eta^ <- ( eta^ - dt L h_i^        ) / ( 1 + dt L kappa_eta |xi|^2 )          (Eqs. 13, 15)
+ * with |xi|^2 of k2_kind. The fields are kept in a partially transformed form between steps; the
+ * real fields are materialised by pf_get_fields / pf_step_fd / pf_free_energy.
+ * nsteps == 0 is a no-op; nsteps < 0 -> PF_EINVAL; no fields set -> PF_ESTATE.
+ * Non-finite values are not an error (they propagate). */
+int pf_step_fs(pf_ctx *ctx, int nsteps);
+
+/* nsteps explicit forward-Euler steps with the 5-point (2D) / 7-point (3D) Laplacian and periodic
+ * wrap-around: mu = df/dc - kappa_c lap c; c += dt M lap mu;
+ * eta_i -= dt L (df/deta_i - kappa_eta lap eta_i); every right-hand side at time t. */
+int pf_step_fd(pf_ctx *ctx, int nsteps);
+
+/* Copies the current fields out (same layouts as pf_set_fields). With PF_HOST the call returns after
+ * the data has arrived. */
+int pf_get_fields(pf_ctx *ctx, void *c, void *eta, int where);
+
+/* Eq. 1 as a Riemann sum with cell volume prod(dx), accumulated in fp64.
+ * out (HOST pointer, 3 + n_eta doubles): total, chemical, kappa_c/2 |grad c|^2, kappa_eta/2 |grad eta_i|^2 ...
+ * gradient_kind 0: spectral, sum_k |xi|^2 |u^_k|^2 / N (Parseval) with the k2_kind frequencies;
+ * gradient_kind 1: forward differences (the discretisation the 5/7-point Laplacian derives from). */
+int pf_free_energy(pf_ctx *ctx, int gradient_kind, double *out);
+
+/* Changes dt for subsequent steps (the dt sweep of the FS-vs-FD crossover); dt <= 0 -> PF_EINVAL. */
+int pf_set_dt(pf_ctx *ctx, double dt);
+
+/* Number of kernel launches (graph kernel nodes included) issued by this context so far. */
+long long pf_launch_count(const pf_ctx *ctx);
+
+/* Device time in milliseconds spent by kernel `which` of the most recent pf_step_fs call, measured
+ * with CUDA events on the context's stream when profiling was switched on with pf_set_profiling
+ * (which = 0 .. pf_num_fs_kernels()-1, in launch order within one step; averaged over the steps of
+ * that call). Returns a negative value when unavailable. Profiling disables CUDA-graph replay. */
+int    pf_set_profiling(pf_ctx *ctx, int on);
+int    pf_num_fs_kernels(const pf_ctx *ctx);
+double pf_fs_kernel_ms(pf_ctx *ctx, int which);
+const char *pf_fs_kernel_name(const pf_ctx *ctx, int which);
+
+const char *pf_strerror(int code);
+const char *pf_last_cuda_error(const pf_ctx *ctx);      /* "" when none */
+
+/* Frees everything the context owns (NULL is allowed). */
+void pf_destroy(pf_ctx *ctx);
+
+#ifdef __cplusplus
+}
+#endif
+#endif

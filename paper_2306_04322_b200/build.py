@@ -1,0 +1,63 @@
+"""Builds libpf.so (the C-ABI library of include/pf.h) in-tree with nvcc for sm_100a.
+
+    python -m paper_2306_04322_b200.build [--force]
+
+The four translation units are compiled in parallel and linked into
+paper_2306_04322_b200/libpf.so (static cudart; no torch, no other dependency).
+"""
+from __future__ import annotations
+
+import os
+import subprocess
+import sys
+from concurrent.futures import ThreadPoolExecutor
+
+HERE = os.path.dirname(os.path.abspath(__file__))
+CSRC = os.path.join(HERE, "csrc")
+OBJ = os.path.join(HERE, "csrc", "build")
+SO = os.path.join(HERE, "libpf.so")
+UNITS = ["row_kernels", "col_kernels", "fd_kernels", "pf"]
+HEADERS = [os.path.join(CSRC, h) for h in ("fft_core.cuh", "pf_kernels.cuh")] + \
+          [os.path.join(os.path.dirname(HERE), "include", "pf.h")]
+NVCC_FLAGS = ["-std=c++17", "-O3", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo",
+              "-Xcompiler", "-fPIC", "-Xptxas", "-v"]
+
+
+def _nvcc() -> str:
+    for cand in (os.environ.get("NVCC"), "/usr/local/cuda/bin/nvcc", "nvcc"):
+        if cand and (os.path.isabs(cand) and os.path.exists(cand) or not os.path.isabs(cand)):
+            return cand
+    return "nvcc"
+
+
+def _stale(target: str, deps) -> bool:
+    if not os.path.exists(target):
+        return True
+    t = os.path.getmtime(target)
+    return any(os.path.getmtime(d) > t for d in deps)
+
+
+def _compile(unit: str, force: bool) -> str:
+    src = os.path.join(CSRC, unit + ".cu")
+    obj = os.path.join(OBJ, unit + ".o")
+    if force or _stale(obj, [src] + HEADERS):
+        log = os.path.join(OBJ, unit + ".ptxas.log")
+        with open(log, "w") as fh:
+            r = subprocess.run([_nvcc()] + NVCC_FLAGS + ["-c", src, "-o", obj], stdout=fh, stderr=subprocess.STDOUT)
+        if r.returncode != 0:
+            sys.stderr.write(open(log).read()[-4000:])
+            raise RuntimeError(f"nvcc failed on {unit}.cu (log: {log})")
+    return obj
+
+
+def build(force: bool = False) -> str:
+    os.makedirs(OBJ, exist_ok=True)
+    with ThreadPoolExecutor(max_workers=len(UNITS)) as ex:
+        objs = list(ex.map(lambda u: _compile(u, force), UNITS))
+    if force or _stale(SO, objs):
+        subprocess.run([_nvcc(), "-shared", "-o", SO] + objs + ["-gencode", "arch=compute_100a,code=sm_100a"], check=True)
+    return SO
+
+
+if __name__ == "__main__":
+    print(build(force="--force" in sys.argv))

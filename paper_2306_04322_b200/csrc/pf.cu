@@ -1,0 +1,541 @@
+// pf.cu -- the C ABI of libpf (include/pf.h): context, buffers, tables, state tracking, launch
+// sequences of the Fourier-spectral and finite-difference steps, CUDA-graph replay.
+//
+// Device data of a context (w = element size, N = nx*ny*nz, M = nx/2, F = 1 + n_eta):
+//   real[2]  [F][nz][ny][nx]        real fields, double buffered (set/get, FD path)
+//   zst      [F][nz][ny][M] complex "z-form" state of the spectral path (row_kernels.cu)
+//   zg       [nz][ny][M]    complex z-form of g = df/dc
+//   s2       [F][nz][ny][P2] complex, 3D only: (kx,ky)-spectral, z-real planes; s2[0] carries c between steps
+//   g2       [nz][ny][P2]   complex, 3D only
+//   mu       [N]            FD chemical potential
+//   tables   twiddles exp(-2 pi i k/n) for M, ny, nz, nx; |xi_d|^2 per axis (Eq. 16-21)
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <new>
+#include <string>
+#include <vector>
+
+#include "../../include/pf.h"
+#include "pf_kernels.cuh"
+
+using namespace pf;
+
+namespace {
+
+enum State { ST_NONE = 0, ST_REAL = 1, ST_SPECTRAL = 2, ST_BOTH = 3 };
+const int kMaxFsKernels = 6;
+
+}  // namespace
+
+struct pf_ctx {
+    pf_params p;
+    int F = 1, M = 0, P2 = 0;
+    long N = 0;
+    size_t w = 8;
+    cudaStream_t stream = nullptr;
+    bool own_stream = false;
+    bool graph_ok = true;
+    void *real[2] = {nullptr, nullptr};
+    int cur = 0;
+    void *zst = nullptr, *zg = nullptr, *s2 = nullptr, *g2 = nullptr, *mu = nullptr;
+    void *tw_m = nullptr, *tw_y = nullptr, *tw_z = nullptr, *tw_nx = nullptr;
+    void *kx2 = nullptr, *ky2 = nullptr, *kz2 = nullptr;
+    double *acc = nullptr;
+    int state = ST_NONE;
+    bool s2c_valid = false;
+    long long launches = 0;
+    std::string cuda_err;
+    // CUDA graph of one FS step
+    cudaGraphExec_t fs_graph = nullptr;
+    int fs_graph_nodes = 0;
+    // profiling
+    bool profiling = false;
+    int nk = 0;
+    const char *kname[kMaxFsKernels] = {};
+    double kms[kMaxFsKernels] = {};
+    cudaEvent_t ev[kMaxFsKernels + 1] = {};
+};
+
+namespace {
+
+#define PF_CK(ctx, call)                                                      \
+    do {                                                                      \
+        cudaError_t e__ = (call);                                             \
+        if (e__ != cudaSuccess) {                                             \
+            (ctx)->cuda_err = std::string(#call) + ": " + cudaGetErrorString(e__); \
+            return e__ == cudaErrorMemoryAllocation ? PF_ENOMEM : PF_ECUDA;   \
+        }                                                                     \
+    } while (0)
+
+bool pow2_in_range(int n) { return n >= 16 && n <= 2048 && (n & (n - 1)) == 0; }
+
+// squared frequency of one axis at index idx:
+//   kind 0: xi^2, xi = 2 pi m / l, m = idx for idx <= n/2 else idx - n          (Eq. 16/19)
+//   kind 1: 2 (1 - cos(dx xi)) / dx^2                                            (Eq. 17/20)
+//   kind 2: (15 - 16 cos(dx xi) + cos(2 dx xi)) / (6 dx^2)                       (Eq. 18/21)
+double axis_k2(int kind, int n, double dx, int idx)
+{
+    const double PI = 3.14159265358979323846264338327950288;
+    const int m = (idx <= n / 2) ? idx : idx - n;
+    const double xi = 2.0 * PI * (double)m / ((double)n * dx);
+    if (kind == 0) return xi * xi;
+    // dx*xi = 2 pi m / n: evaluate the cosine of the exact rational angle
+    const double a = 2.0 * PI * (double)m / (double)n;
+    if (kind == 1) return 2.0 * (1.0 - std::cos(a)) / (dx * dx);
+    return (15.0 - 16.0 * std::cos(a) + std::cos(2.0 * a)) / (6.0 * dx * dx);
+}
+
+template <typename T> Model<T> make_model(const pf_params &p)
+{
+    Model<T> m;
+    m.rho2 = (T)p.rho2; m.c_alpha = (T)p.c_alpha; m.c_beta = (T)p.c_beta; m.w = (T)p.w; m.alpha = (T)p.alpha;
+    m.kappa_c = (T)p.kappa_c; m.kappa_eta = (T)p.kappa_eta;
+    m.dt = (T)p.dt; m.M = (T)p.M; m.L = (T)p.L;
+    m.dtM = (T)(p.dt * p.M); m.dtL = (T)(p.dt * p.L);
+    m.dtMkc = (T)(p.dt * p.M * p.kappa_c); m.dtLke = (T)(p.dt * p.L * p.kappa_eta);
+    m.n_eta = p.n_eta;
+    return m;
+}
+
+template <typename T> int upload_tables(pf_ctx *c)
+{
+    typedef typename V2<T>::type C;
+    const long double PI = 3.141592653589793238462643383279502884L;
+    auto twiddles = [&](int n, int count, void **dst) -> int {
+        std::vector<C> h(count);
+        for (int k = 0; k < count; ++k) {
+            // reduce to the first octant for full accuracy at every k
+            h[k].x = (T)cosl(2 * PI * (long double)k / n);
+            h[k].y = (T)-sinl(2 * PI * (long double)k / n);
+        }
+        PF_CK(c, cudaMalloc(dst, sizeof(C) * count));
+        PF_CK(c, cudaMemcpy(*dst, h.data(), sizeof(C) * count, cudaMemcpyHostToDevice));
+        return PF_OK;
+    };
+    int rc;
+    if ((rc = twiddles(c->M, c->M, &c->tw_m))) return rc;
+    if ((rc = twiddles(c->p.n[1], c->p.n[1], &c->tw_y))) return rc;
+    if ((rc = twiddles(c->p.n[2] > 1 ? c->p.n[2] : 2, c->p.n[2] > 1 ? c->p.n[2] : 2, &c->tw_z))) return rc;
+    if ((rc = twiddles(c->p.n[0], c->M + 1, &c->tw_nx))) return rc;
+    auto ktable = [&](int axis, int count, int padded, void **dst) -> int {
+        std::vector<T> h(padded, (T)0);
+        for (int k = 0; k < count; ++k) h[k] = (T)axis_k2(c->p.k2_kind, c->p.n[axis], c->p.dx[axis], k);
+        PF_CK(c, cudaMalloc(dst, sizeof(T) * padded));
+        PF_CK(c, cudaMemcpy(*dst, h.data(), sizeof(T) * padded, cudaMemcpyHostToDevice));
+        return PF_OK;
+    };
+    if ((rc = ktable(0, c->M + 1, c->P2, &c->kx2))) return rc;
+    if ((rc = ktable(1, c->p.n[1], c->p.n[1], &c->ky2))) return rc;
+    if (c->p.ndim == 3) { if ((rc = ktable(2, c->p.n[2], c->p.n[2], &c->kz2))) return rc; }
+    else {
+        PF_CK(c, cudaMalloc(&c->kz2, sizeof(T) * 2));
+        PF_CK(c, cudaMemset(c->kz2, 0, sizeof(T) * 2));
+    }
+    return PF_OK;
+}
+
+void drop_graph(pf_ctx *c)
+{
+    if (c->fs_graph) { cudaGraphExecDestroy(c->fs_graph); c->fs_graph = nullptr; }
+}
+
+// ---------------------------------------------------------------- launch sequences ----------------
+template <typename T> RowParams<T> row_params(pf_ctx *c)
+{
+    typedef typename V2<T>::type C;
+    RowParams<T> r;
+    r.zst = (C *)c->zst; r.zg = (C *)c->zg; r.real = (T *)c->real[c->cur];
+    r.tw = (const C *)c->tw_m;
+    r.zfs = c->N / 2; r.rfs = c->N;
+    r.nrows = c->p.n[1] * c->p.n[2]; r.F = c->F;
+    r.m = make_model<T>(c->p);
+    return r;
+}
+
+template <typename T> ColParams<T> col_params(pf_ctx *c)
+{
+    typedef typename V2<T>::type C;
+    ColParams<T> q;
+    memset(&q, 0, sizeof(q));
+    q.M = c->M; q.P2 = c->P2;
+    q.twx = (const C *)c->tw_nx;
+    q.kx2 = (const T *)c->kx2; q.ky2 = (const T *)c->ky2; q.kz2 = (const T *)c->kz2;
+    q.acc = c->acc;
+    q.m = make_model<T>(c->p);
+    return q;
+}
+
+struct KernelTimer {
+    pf_ctx *c; int k = 0;
+    explicit KernelTimer(pf_ctx *ctx) : c(ctx) { if (c->profiling) cudaEventRecord(c->ev[0], c->stream); }
+    void mark(const char *name)
+    {
+        if (k < kMaxFsKernels) { c->kname[k] = name; if (c->profiling) cudaEventRecord(c->ev[k + 1], c->stream); ++k; }
+    }
+};
+
+// 3D: (kx,ky)-spectral planes of the listed z-form fields: s2[f] (or g2) <- FFT_y(unpack(z-form))
+template <typename T> cudaError_t mid_forward(pf_ctx *c, const void *zsrc, long zfs, void *dst, long dfs, int nfields)
+{
+    typedef typename V2<T>::type C;
+    const int ny = c->p.n[1], nz = c->p.n[2];
+    ColParams<T> q = col_params<T>(c);
+    q.in0 = (const C *)zsrc; q.in_fs = zfs; q.in_rs = c->M; q.in_bs = (long)ny * c->M;
+    q.out = (C *)dst; q.out_fs = dfs; q.out_rs = c->P2; q.out_bs = (long)ny * c->P2;
+    q.tw = (const C *)c->tw_y;
+    ++c->launches;
+    return launch_col<T>(COL_3D_MIDFWD, false, ny, nfields, nz, q, c->stream);
+}
+
+template <typename T> int fs_one_step(pf_ctx *c)
+{
+    typedef typename V2<T>::type C;
+    const int ny = c->p.n[1], nz = c->p.n[2], p = c->p.n_eta;
+    const long zfs = c->N / 2;
+    KernelTimer kt(c);
+    RowParams<T> r = row_params<T>(c);
+    PF_CK(c, launch_row<T>(ROW_STEP, c->p.n[0], r, c->stream)); ++c->launches; kt.mark("row_c2r_nonlinear_r2c");
+    C *zst = (C *)c->zst;
+    if (c->p.ndim == 2) {
+        ColParams<T> q = col_params<T>(c);
+        q.tw = (const C *)c->tw_y;
+        q.in_rs = q.out_rs = c->M;
+        q.in0 = zst; q.in1 = (const C *)c->zg; q.out = zst;
+        PF_CK(c, launch_col<T>(COL_2D_LAST, true, ny, 1, 1, q, c->stream)); ++c->launches; kt.mark("col_y_update_c");
+        if (p > 0) {
+            q.in0 = zst + zfs; q.out = zst + zfs; q.in_fs = q.out_fs = zfs; q.in1 = nullptr;
+            PF_CK(c, launch_col<T>(COL_2D_LAST, false, ny, p, 1, q, c->stream)); ++c->launches; kt.mark("col_y_update_eta");
+        }
+    } else {
+        const long s2fs = (long)nz * ny * c->P2;
+        C *s2 = (C *)c->s2;
+        PF_CK(c, mid_forward<T>(c, c->zg, 0, c->g2, 0, 1)); kt.mark("col_y_fwd_g");
+        if (p > 0) { PF_CK(c, mid_forward<T>(c, zst + zfs, zfs, s2 + s2fs, s2fs, p)); kt.mark("col_y_fwd_eta"); }
+        ColParams<T> q = col_params<T>(c);
+        q.tw = (const C *)c->tw_z;
+        q.in_rs = q.out_rs = (long)ny * c->P2; q.ncols = ny * c->P2;
+        q.in0 = s2; q.in1 = (const C *)c->g2; q.out = s2;
+        PF_CK(c, launch_col<T>(COL_3D_LAST, true, nz, 1, 1, q, c->stream)); ++c->launches; kt.mark("col_z_update_c");
+        if (p > 0) {
+            q.in0 = s2 + s2fs; q.out = s2 + s2fs; q.in_fs = q.out_fs = s2fs; q.in1 = nullptr;
+            PF_CK(c, launch_col<T>(COL_3D_LAST, false, nz, p, 1, q, c->stream)); ++c->launches; kt.mark("col_z_update_eta");
+        }
+        ColParams<T> v = col_params<T>(c);
+        v.tw = (const C *)c->tw_y;
+        v.in0 = s2; v.in_fs = s2fs; v.in_rs = c->P2; v.in_bs = (long)ny * c->P2;
+        v.out = zst; v.out_fs = zfs; v.out_rs = c->M; v.out_bs = (long)ny * c->M;
+        PF_CK(c, launch_col<T>(COL_3D_MIDINV, false, ny, c->F, nz, v, c->stream)); ++c->launches; kt.mark("col_y_inv");
+    }
+    c->nk = kt.k;
+    return PF_OK;
+}
+
+// real fields -> z-form state (and, in 3D, the carried (kx,ky)-spectral planes of c)
+template <typename T> int to_spectral(pf_ctx *c)
+{
+    if (c->state == ST_REAL) {
+        RowParams<T> r = row_params<T>(c);
+        PF_CK(c, launch_row<T>(ROW_SET, c->p.n[0], r, c->stream)); ++c->launches;
+        c->state = ST_BOTH;
+    }
+    if (c->p.ndim == 3 && !c->s2c_valid) {
+        PF_CK(c, mid_forward<T>(c, c->zst, 0, c->s2, 0, 1));
+        c->s2c_valid = true;
+    }
+    return PF_OK;
+}
+
+template <typename T> int to_real(pf_ctx *c)
+{
+    if (c->state == ST_SPECTRAL) {
+        RowParams<T> r = row_params<T>(c);
+        PF_CK(c, launch_row<T>(ROW_GET, c->p.n[0], r, c->stream)); ++c->launches;
+        c->state = ST_BOTH;
+    }
+    return PF_OK;
+}
+
+template <typename T> int step_fs(pf_ctx *c, int nsteps)
+{
+    int rc = to_spectral<T>(c);
+    if (rc) return rc;
+    if (c->profiling) {
+        double sum[kMaxFsKernels] = {};
+        for (int s = 0; s < nsteps; ++s) {
+            if ((rc = fs_one_step<T>(c))) return rc;
+            PF_CK(c, cudaEventSynchronize(c->ev[c->nk]));
+            for (int k = 0; k < c->nk; ++k) { float ms = 0; cudaEventElapsedTime(&ms, c->ev[k], c->ev[k + 1]); sum[k] += ms; }
+        }
+        for (int k = 0; k < c->nk; ++k) c->kms[k] = sum[k] / nsteps;
+    } else {
+        // replay one captured step; small grids are launch-latency bound without it
+        if (!c->fs_graph && c->graph_ok && nsteps >= 2) {
+            cudaGraph_t g = nullptr;
+            const long long before = c->launches;
+            if (cudaStreamBeginCapture(c->stream, cudaStreamCaptureModeThreadLocal) == cudaSuccess) {
+                rc = fs_one_step<T>(c);
+                cudaError_t e = cudaStreamEndCapture(c->stream, &g);
+                c->fs_graph_nodes = (int)(c->launches - before);
+                c->launches = before;
+                if (rc) { if (g) cudaGraphDestroy(g); return rc; }
+                PF_CK(c, e);
+                e = cudaGraphInstantiate(&c->fs_graph, g, 0);
+                cudaGraphDestroy(g);
+                PF_CK(c, e);
+            } else {
+                cudaGetLastError();          // a stream that cannot be captured: plain launches
+                c->graph_ok = false;
+            }
+        }
+        for (int s = 0; s < nsteps; ++s) {
+            if (c->fs_graph) { PF_CK(c, cudaGraphLaunch(c->fs_graph, c->stream)); c->launches += c->fs_graph_nodes; }
+            else if ((rc = fs_one_step<T>(c))) return rc;
+        }
+    }
+    c->state = ST_SPECTRAL;
+    return PF_OK;
+}
+
+template <typename T> int step_fd(pf_ctx *c, int nsteps)
+{
+    int rc = to_real<T>(c);
+    if (rc) return rc;
+    FdParams<T> f;
+    f.nx = c->p.n[0]; f.ny = c->p.n[1]; f.nz = c->p.n[2]; f.N = c->N;
+    for (int d = 0; d < 3; ++d) f.rdx2[d] = (d < c->p.ndim) ? (T)(1.0 / (c->p.dx[d] * c->p.dx[d])) : (T)0;
+    f.m = make_model<T>(c->p);
+    f.mu = (T *)c->mu;
+    for (int s = 0; s < nsteps; ++s) {
+        T *cu = (T *)c->real[c->cur], *nw = (T *)c->real[c->cur ^ 1];
+        f.c = cu; f.eta = cu + c->N; f.c_new = nw; f.eta_new = nw + c->N;
+        PF_CK(c, launch_fd_mu<T>(f, c->stream));
+        PF_CK(c, launch_fd_update<T>(f, c->stream));
+        c->launches += 2;
+        c->cur ^= 1;
+    }
+    c->state = ST_REAL;
+    c->s2c_valid = false;
+    return PF_OK;
+}
+
+template <typename T> int free_energy(pf_ctx *c, int kind, double *out)
+{
+    typedef typename V2<T>::type C;
+    int rc = to_real<T>(c);
+    if (rc) return rc;
+    const int p = c->p.n_eta, nacc = 2 + p;
+    PF_CK(c, cudaMemsetAsync(c->acc, 0, sizeof(double) * 32, c->stream));
+    EnergyParams<T> e;
+    e.c = (const T *)c->real[c->cur]; e.eta = e.c + c->N;
+    e.nx = c->p.n[0]; e.ny = c->p.n[1]; e.nz = c->p.n[2]; e.N = c->N;
+    for (int d = 0; d < 3; ++d) e.rdx[d] = (d < c->p.ndim) ? (T)(1.0 / c->p.dx[d]) : (T)0;
+    e.gradient_kind = kind; e.acc = c->acc; e.m = make_model<T>(c->p);
+    PF_CK(c, launch_energy<T>(e, c->stream)); ++c->launches;
+    double scale_grad = 1.0;
+    if (kind == 0) {
+        // Parseval: sum_x |grad u|^2 = (1/N) sum_k |xi|^2 |u^_k|^2
+        if ((rc = to_spectral<T>(c))) return rc;
+        ColParams<T> q = col_params<T>(c);
+        q.acc = c->acc + 1;
+        const int ny = c->p.n[1], nz = c->p.n[2];
+        if (c->p.ndim == 2) {
+            q.tw = (const C *)c->tw_y; q.in0 = (const C *)c->zst; q.in_fs = c->N / 2; q.in_rs = c->M;
+            PF_CK(c, launch_col<T>(COL_2D_ENERGY, false, ny, c->F, 1, q, c->stream)); ++c->launches;
+        } else {
+            const long s2fs = (long)nz * ny * c->P2;
+            if (p > 0) PF_CK(c, mid_forward<T>(c, (C *)c->zst + c->N / 2, c->N / 2, (C *)c->s2 + s2fs, s2fs, p));
+            q.tw = (const C *)c->tw_z; q.in0 = (const C *)c->s2; q.in_fs = s2fs; q.in_rs = (long)ny * c->P2;
+            q.ncols = ny * c->P2;
+            PF_CK(c, launch_col<T>(COL_3D_ENERGY, false, nz, c->F, 1, q, c->stream)); ++c->launches;
+        }
+        scale_grad = 1.0 / (double)c->N;
+    }
+    double h[32];
+    PF_CK(c, cudaMemcpyAsync(h, c->acc, sizeof(double) * nacc, cudaMemcpyDeviceToHost, c->stream));
+    PF_CK(c, cudaStreamSynchronize(c->stream));
+    double dV = 1.0;
+    for (int d = 0; d < c->p.ndim; ++d) dV *= c->p.dx[d];
+    out[1] = h[0] * dV;
+    out[2] = 0.5 * c->p.kappa_c * h[1] * scale_grad * dV;
+    double tot = out[1] + out[2];
+    for (int k = 0; k < p; ++k) { out[3 + k] = 0.5 * c->p.kappa_eta * h[2 + k] * scale_grad * dV; tot += out[3 + k]; }
+    out[0] = tot;
+    return PF_OK;
+}
+
+int copy_fields(pf_ctx *c, void *dc, void *deta, const void *sc, const void *seta, cudaMemcpyKind kind)
+{
+    const size_t fb = (size_t)c->N * c->w;
+    PF_CK(c, cudaMemcpyAsync(dc, sc, fb, kind, c->stream));
+    if (c->p.n_eta > 0) PF_CK(c, cudaMemcpyAsync(deta, seta, fb * c->p.n_eta, kind, c->stream));
+    return PF_OK;
+}
+
+}  // namespace
+
+// ================================================================== C ABI =========================
+extern "C" {
+
+const char *pf_strerror(int code)
+{
+    switch (code) {
+    case PF_OK: return "ok";
+    case PF_EINVAL: return "invalid argument";
+    case PF_ENOMEM: return "out of device memory";
+    case PF_ECUDA: return "CUDA error";
+    case PF_ESTATE: return "no fields set";
+    case PF_EUNSUPPORTED: return "unsupported grid size";
+    }
+    return "unknown error";
+}
+
+const char *pf_last_cuda_error(const pf_ctx *ctx) { return ctx ? ctx->cuda_err.c_str() : ""; }
+
+void pf_destroy(pf_ctx *c)
+{
+    if (!c) return;
+    drop_graph(c);
+    for (auto &e : c->ev) if (e) cudaEventDestroy(e);
+    void *bufs[] = {c->real[0], c->real[1], c->zst, c->zg, c->s2, c->g2, c->mu, c->tw_m, c->tw_y, c->tw_z,
+                    c->tw_nx, c->kx2, c->ky2, c->kz2, c->acc};
+    for (void *b : bufs) if (b) cudaFree(b);
+    if (c->own_stream) cudaStreamDestroy(c->stream);
+    delete c;
+}
+
+int pf_create(const pf_params *p, pf_ctx **out)
+{
+    if (!p || !out) return PF_EINVAL;
+    if (p->ndim != 2 && p->ndim != 3) return PF_EINVAL;
+    if (p->n_eta < 0 || p->n_eta > 8) return PF_EINVAL;
+    if (!(p->dt > 0.0)) return PF_EINVAL;
+    if (p->precision != PF_F32 && p->precision != PF_F64) return PF_EINVAL;
+    if (p->k2_kind < 0 || p->k2_kind > 2) return PF_EINVAL;
+    for (int d = 0; d < p->ndim; ++d) if (!(p->dx[d] > 0.0)) return PF_EINVAL;
+    for (int d = 0; d < p->ndim; ++d) if (!pow2_in_range(p->n[d])) return PF_EUNSUPPORTED;
+    if (p->ndim == 2 && p->n[2] != 1) return PF_EUNSUPPORTED;
+
+    int ndev = 0;
+    if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev <= 0) { cudaGetLastError(); return PF_ECUDA; }
+
+    pf_ctx *c = new (std::nothrow) pf_ctx();
+    if (!c) return PF_ENOMEM;
+    c->p = *p;
+    if (p->ndim == 2) { c->p.n[2] = 1; c->p.dx[2] = 1.0; }
+    c->F = 1 + p->n_eta;
+    c->M = p->n[0] / 2;
+    c->P2 = ((c->M + 1 + 15) / 16) * 16;
+    c->N = (long)c->p.n[0] * c->p.n[1] * c->p.n[2];
+    c->w = (p->precision == PF_F64) ? 8 : 4;
+    c->stream = (cudaStream_t)p->stream;
+    if (!c->stream) {
+        // NULL: a private blocking stream (ordered with the legacy default stream, and capturable)
+        if (cudaStreamCreate(&c->stream) != cudaSuccess) { cudaGetLastError(); delete c; return PF_ECUDA; }
+        c->own_stream = true;
+    }
+
+    auto fail = [&](int rc) { pf_destroy(c); return rc; };
+    auto alloc = [&](void **dst, size_t bytes) -> int {
+        cudaError_t e = cudaMalloc(dst, bytes);
+        if (e != cudaSuccess) { cudaGetLastError(); return e == cudaErrorMemoryAllocation ? PF_ENOMEM : PF_ECUDA; }
+        e = cudaMemset(*dst, 0, bytes);
+        return e == cudaSuccess ? PF_OK : PF_ECUDA;
+    };
+    const size_t fb = (size_t)c->N * c->w;                 // one real field
+    int rc;
+    if ((rc = alloc(&c->real[0], fb * c->F)) || (rc = alloc(&c->real[1], fb * c->F)) ||
+        (rc = alloc(&c->zst, fb * c->F)) || (rc = alloc(&c->zg, fb)) || (rc = alloc(&c->mu, fb)) ||
+        (rc = alloc((void **)&c->acc, sizeof(double) * 32)))
+        return fail(rc);
+    if (p->ndim == 3) {
+        const size_t pb = (size_t)c->p.n[2] * c->p.n[1] * c->P2 * 2 * c->w;
+        if ((rc = alloc(&c->s2, pb * c->F)) || (rc = alloc(&c->g2, pb))) return fail(rc);
+    }
+    rc = (p->precision == PF_F64) ? upload_tables<double>(c) : upload_tables<float>(c);
+    if (rc) return fail(rc);
+    for (auto &e : c->ev) if (cudaEventCreate(&e) != cudaSuccess) return fail(PF_ECUDA);
+    *out = c;
+    return PF_OK;
+}
+
+int pf_set_fields(pf_ctx *c, const void *fc, const void *eta, int where)
+{
+    if (!c || !fc || (c->p.n_eta > 0 && !eta)) return PF_EINVAL;
+    if (where != PF_HOST && where != PF_DEVICE) return PF_EINVAL;
+    char *dst = (char *)c->real[c->cur];
+    int rc = copy_fields(c, dst, dst + (size_t)c->N * c->w, fc, eta,
+                         where == PF_HOST ? cudaMemcpyHostToDevice : cudaMemcpyDeviceToDevice);
+    if (rc) return rc;
+    if (where == PF_HOST) PF_CK(c, cudaStreamSynchronize(c->stream));
+    c->state = ST_REAL;
+    c->s2c_valid = false;
+    return PF_OK;
+}
+
+int pf_get_fields(pf_ctx *c, void *fc, void *eta, int where)
+{
+    if (!c || !fc || (c->p.n_eta > 0 && !eta)) return PF_EINVAL;
+    if (where != PF_HOST && where != PF_DEVICE) return PF_EINVAL;
+    if (c->state == ST_NONE) return PF_ESTATE;
+    int rc = (c->p.precision == PF_F64) ? to_real<double>(c) : to_real<float>(c);
+    if (rc) return rc;
+    const char *src = (const char *)c->real[c->cur];
+    rc = copy_fields(c, fc, eta, src, src + (size_t)c->N * c->w,
+                     where == PF_HOST ? cudaMemcpyDeviceToHost : cudaMemcpyDeviceToDevice);
+    if (rc) return rc;
+    if (where == PF_HOST) PF_CK(c, cudaStreamSynchronize(c->stream));
+    return PF_OK;
+}
+
+int pf_step_fs(pf_ctx *c, int nsteps)
+{
+    if (!c || nsteps < 0) return PF_EINVAL;
+    if (c->state == ST_NONE) return PF_ESTATE;
+    if (nsteps == 0) return PF_OK;
+    return (c->p.precision == PF_F64) ? step_fs<double>(c, nsteps) : step_fs<float>(c, nsteps);
+}
+
+int pf_step_fd(pf_ctx *c, int nsteps)
+{
+    if (!c || nsteps < 0) return PF_EINVAL;
+    if (c->state == ST_NONE) return PF_ESTATE;
+    if (nsteps == 0) return PF_OK;
+    return (c->p.precision == PF_F64) ? step_fd<double>(c, nsteps) : step_fd<float>(c, nsteps);
+}
+
+int pf_free_energy(pf_ctx *c, int gradient_kind, double *out)
+{
+    if (!c || !out || (gradient_kind != 0 && gradient_kind != 1)) return PF_EINVAL;
+    if (c->state == ST_NONE) return PF_ESTATE;
+    return (c->p.precision == PF_F64) ? free_energy<double>(c, gradient_kind, out)
+                                      : free_energy<float>(c, gradient_kind, out);
+}
+
+int pf_set_dt(pf_ctx *c, double dt)
+{
+    if (!c || !(dt > 0.0)) return PF_EINVAL;
+    c->p.dt = dt;
+    drop_graph(c);                       // dt is baked into the captured kernel arguments
+    return PF_OK;
+}
+
+long long pf_launch_count(const pf_ctx *c) { return c ? c->launches : 0; }
+
+int pf_set_profiling(pf_ctx *c, int on)
+{
+    if (!c) return PF_EINVAL;
+    c->profiling = on != 0;
+    for (double &v : c->kms) v = -1.0;
+    return PF_OK;
+}
+int pf_num_fs_kernels(const pf_ctx *c)
+{
+    if (!c) return 0;
+    const int e = c->p.n_eta > 0 ? 1 : 0;
+    return c->p.ndim == 2 ? 2 + e : 4 + 2 * e;
+}
+double pf_fs_kernel_ms(pf_ctx *c, int which) { return (c && which >= 0 && which < c->nk) ? c->kms[which] : -1.0; }
+const char *pf_fs_kernel_name(const pf_ctx *c, int which) { return (c && which >= 0 && which < c->nk && c->kname[which]) ? c->kname[which] : ""; }
+
+}  // extern "C"

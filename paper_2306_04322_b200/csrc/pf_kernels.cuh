@@ -1,0 +1,115 @@
+// pf_kernels.cuh -- parameter blocks and launch entry points shared by the kernel translation units
+// and the host library (pf.cu). Product code; nothing here is shared with oracle/.
+#pragma once
+#include <cuda_runtime.h>
+#include "fft_core.cuh"
+
+namespace pf {
+
+// Model coefficients in the arithmetic type of the kernels (Eqs. 1-3, 12-15).
+template <typename T> struct Model {
+    T rho2, c_alpha, c_beta, w, alpha;     // f_chem
+    T kappa_c, kappa_eta;
+    T dt, M, L;
+    T dtM, dtL;                            // dt*M, dt*L            (Eqs. 12-13)
+    T dtMkc, dtLke;                        // dt*M*kappa_c, dt*L*kappa_eta   (Eqs. 14-15)
+    int n_eta;
+};
+
+enum RowMode { ROW_SET = 0, ROW_STEP = 1, ROW_GET = 2 };
+
+// x-direction kernel. "z-form" of a real row u[0..nx): Z = FFT_{nx/2}( u[2n] + i u[2n+1] ), nx/2 complex values.
+template <typename T> struct RowParams {
+    typedef typename V2<T>::type C;
+    C       *zst;            // [F][nrows][M]   state, z-form (M = nx/2)
+    C       *zg;             // [nrows][M]      z-form of g = df_chem/dc (ROW_STEP output)
+    T       *real;           // [F][nrows][nx]  real fields (ROW_SET input / ROW_GET output)
+    const C *tw;             // exp(-2 pi i k / M), k < M
+    long     zfs;            // field stride of zst in complex elements (= nrows*M)
+    long     rfs;            // field stride of real in reals (= nrows*nx)
+    int      nrows;          // ny*nz
+    int      F;              // 1 + n_eta
+    Model<T> m;
+};
+
+// Column-kernel modes (see col_kernels.cu)
+enum ColMode {
+    COL_2D_LAST   = 0,   // z-form pairs -> unpack, FFT_y, spectral update, IFFT_y, repack -> z-form
+    COL_3D_MIDFWD = 1,   // z-form pairs -> unpack, FFT_y -> half-spectrum planes [nz][ny][P2]
+    COL_3D_MIDINV = 2,   // half-spectrum planes -> IFFT_y, repack -> z-form
+    COL_3D_LAST   = 3,   // half-spectrum columns along z: FFT_z, spectral update, IFFT_z (in place)
+    COL_2D_ENERGY = 4,   // z-form pairs -> unpack, FFT_y, accumulate sum w_k |xi|^2 |u^|^2
+    COL_3D_ENERGY = 5    // half-spectrum columns along z: FFT_z, accumulate
+};
+
+template <typename T> struct ColParams {
+    typedef typename V2<T>::type C;
+    const C *in0;            // primary input  (eta fields: w = eta - dt L h; c field: the state u)
+    const C *in1;            // c field only: g = df/dc
+    C       *out;
+    long     in_fs, in1_fs, out_fs;   // field strides (blockIdx.z)
+    long     in_bs, out_bs;           // batch strides (blockIdx.y; 3D mid kernels: z planes)
+    long     in_rs, out_rs;           // stride between consecutive elements along the FFT axis
+    int      M;              // nx/2
+    int      P2;             // pitch of half-spectrum planes (>= M+1, multiple of 8)
+    int      ncols;          // plain-column modes: number of columns (3D last: ny*P2)
+    const C *tw;             // exp(-2 pi i k / N), N = length of the FFT axis
+    const C *twx;            // exp(-2 pi i k / nx), k <= M/2   (Hermitian pack/unpack)
+    const T *kx2;            // |xi_x|^2 per kx, P2 entries (zero padded)
+    const T *ky2;            // per ky (2D last: the FFT axis; 3D last: the middle axis)
+    const T *kz2;            // per kz (3D last: the FFT axis)
+    double  *acc;            // energy modes: accumulator (one double per field)
+    Model<T> m;
+};
+
+// FD path
+template <typename T> struct FdParams {
+    const T *c, *eta;        // time-t fields
+    T       *mu;             // chemical potential scratch
+    T       *c_new, *eta_new;
+    int      nx, ny, nz;
+    long     N;              // nx*ny*nz
+    T        rdx2[3];        // 1/dx^2 per axis (rdx2[2] = 0 in 2D)
+    Model<T> m;
+};
+
+template <typename T> struct EnergyParams {
+    const T *c, *eta;
+    int      nx, ny, nz;
+    long     N;
+    T        rdx[3];         // 1/dx per axis (0 in z for 2D)
+    int      gradient_kind;  // 1: add forward-difference gradient terms; 0: chemical part only
+    double  *acc;            // [2 + n_eta]: chem, grad c, grad eta_i
+    Model<T> m;
+};
+
+// ---- launchers (defined in the .cu files; return cudaGetLastError()) ----
+template <typename T> cudaError_t launch_row(int mode, int nx, const RowParams<T> &p, cudaStream_t s);
+template <typename T> cudaError_t launch_col(int mode, bool is_c, int nfft, int nfields, int nbatch,
+                                             const ColParams<T> &p, cudaStream_t s);
+template <typename T> cudaError_t launch_fd_mu(const FdParams<T> &p, cudaStream_t s);
+template <typename T> cudaError_t launch_fd_update(const FdParams<T> &p, cudaStream_t s);
+template <typename T> cudaError_t launch_energy(const EnergyParams<T> &p, cudaStream_t s);
+
+// pointwise model, shared by the row kernel, the FD kernels and the energy kernel --------------------
+// h(eta) = sum eta^3 (6 eta^2 - 15 eta + 10); g(eta) = sum eta^2 (1-eta)^2 + alpha sum_i sum_{j!=i} eta_i^2 eta_j^2
+// f_chem = rho2 (c-c_alpha)^2 (1-h) + rho2 (c_beta-c)^2 h + w g
+template <typename T> PF_HD T h_term(T e) { return e * e * e * (e * (T(6) * e - T(15)) + T(10)); }
+// d f_chem / dc = 2 rho2 [ (c - c_alpha)(1 - h) - (c_beta - c) h ]
+template <typename T> PF_HD T dfdc(const Model<T> &m, T c, T h)
+{
+    return T(2) * m.rho2 * ((c - m.c_alpha) * (T(1) - h) - (m.c_beta - c) * h);
+}
+// d f_chem / d eta_i = (f^beta - f^alpha) 30 eta^2 (1-eta)^2 + w [ 2 eta (1-eta)(1-2 eta) + 4 alpha eta (s2 - eta^2) ],
+// s2 = sum_j eta_j^2 (each unordered pair appears twice in the ordered double sum of g -> 4 alpha)
+template <typename T> PF_HD T dfdeta(const Model<T> &m, T c, T e, T s2)
+{
+    const T da = c - m.c_alpha, db = m.c_beta - c;
+    const T fba = m.rho2 * (db * db - da * da);
+    const T ome = T(1) - e;
+    const T dh = T(30) * e * e * ome * ome;
+    const T dg = T(2) * e * ome * (T(1) - T(2) * e) + T(4) * m.alpha * e * (s2 - e * e);
+    return fba * dh + m.w * dg;
+}
+
+}  // namespace pf

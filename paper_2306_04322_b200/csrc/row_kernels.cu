@@ -1,0 +1,165 @@
+// row_kernels.cu -- the x-direction kernel of the Fourier-spectral step.
+//
+// State between steps is the "z-form": for every grid row (fixed y, z) and field, the length-M = nx/2
+// complex transform of the packed row  z[n] = u[2n] + i u[2n+1].  The Hermitian split that turns it
+// into the true half spectrum is pointwise in y and lives in the column kernels, so this kernel is
+// pure complex FFT work:
+//
+//   ROW_STEP:  load z-form of c, eta_1..p      -> inverse FFT_M -> real samples c, eta_i (registers)
+//              -> share the samples of the F fields of the row through shared memory
+//              -> g = df_chem/dc                                (Alg. 1; f_chem PAPER.md:46)
+//                 w_i = eta_i - dt L df_chem/deta_i             (right-hand side of Eq. 13, PAPER.md:107,
+//                                                                formed in real space: F is linear)
+//              -> forward FFT_M -> store z-form of g (own array) and of w_i (over eta_i's state)
+//   ROW_SET:   real fields -> forward FFT_M -> z-form state
+//   ROW_GET:   z-form state -> inverse FFT_M / M -> real fields
+//
+// Thread layout: block = RB rows x F fields x TT = M/E threads; thread (r, f, j) owns elements
+// j + q*TT of the transform of field f of row r (fft_core.cuh). One barrier-separated shared-memory
+// exchange per FFT stage boundary plus one for the nonlinear coupling.
+#include "pf_kernels.cuh"
+
+namespace pf {
+
+template <typename C, int LOGPAD> struct RowBuf {
+    C *base;
+    __device__ __forceinline__ void st(int i, C v) { base[i + (i >> LOGPAD)] = v; }
+    __device__ __forceinline__ C ld(int i) const { return base[i + (i >> LOGPAD)]; }
+};
+struct CtaSync { __device__ __forceinline__ void operator()() const { __syncthreads(); } };
+
+template <int M, int E> __host__ __device__ constexpr int row_pitch() { return M + (M >> 3) + 1; }
+
+template <typename T, int M, int E, int MODE>
+__global__ void row_kernel(const RowParams<T> p)
+{
+    typedef typename V2<T>::type C;
+    constexpr int TT = M / E;
+    constexpr int MP = row_pitch<M, E>();
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    C *smem = reinterpret_cast<C *>(smem_raw);
+
+    const int F = p.F;
+    const int tid = threadIdx.x;
+    const int j = tid & (TT - 1);
+    const int rf = tid / TT;
+    const int r = rf / F;
+    const int f = rf - r * F;
+    const int RB = blockDim.x / (TT * F);
+    const long row = (long)blockIdx.x * RB + r;
+    const bool valid = row < p.nrows;
+    RowBuf<C, 3> buf{smem + (long)rf * MP};
+    CtaSync sync;
+
+    C v[E];
+    if (MODE == ROW_SET) {
+        const C *src = reinterpret_cast<const C *>(p.real + f * p.rfs + row * (2L * M));
+#pragma unroll
+        for (int q = 0; q < E; ++q) v[q] = valid ? src[j + q * TT] : mk<T>(0, 0);
+    } else {
+        const C *src = p.zst + f * p.zfs + row * M;
+#pragma unroll
+        for (int q = 0; q < E; ++q) v[q] = valid ? cswap(src[j + q * TT]) : mk<T>(0, 0);   // swap: inverse via forward
+        fft_stages<M, E, 1>(v, j, p.tw, buf, sync);
+        const T s = T(1) / T(M);
+#pragma unroll
+        for (int q = 0; q < E; ++q) v[q] = mk<T>(v[q].y * s, v[q].x * s);                    // swap back, normalise
+    }
+
+    if (MODE == ROW_GET) {
+        C *dst = reinterpret_cast<C *>(p.real + f * p.rfs + row * (2L * M));
+        if (valid) {
+#pragma unroll
+            for (int q = 0; q < E; ++q) dst[j + q * TT] = v[q];
+        }
+        return;
+    }
+
+    if (MODE == ROW_STEP) {
+        // v[q] = (u_f[2n], u_f[2n+1]) at n = j + q*TT. Share across the fields of the row.
+        sync();
+#pragma unroll
+        for (int q = 0; q < E; ++q) buf.st(j + q * TT, v[q]);
+        sync();
+        const C *rowbase = smem + (long)(r * F) * MP;
+#pragma unroll
+        for (int q = 0; q < E; ++q) {
+            const int n = j + q * TT;
+            const int np = n + (n >> 3);
+            T h0 = 0, h1 = 0, s0 = 0, s1 = 0;
+            for (int ff = 1; ff < F; ++ff) {
+                const C e = rowbase[(long)ff * MP + np];
+                h0 += h_term(e.x); h1 += h_term(e.y);
+                s0 += e.x * e.x;   s1 += e.y * e.y;
+            }
+            if (f == 0) {
+                v[q] = mk<T>(dfdc(p.m, v[q].x, h0), dfdc(p.m, v[q].y, h1));
+            } else {
+                const C c = rowbase[np];
+                v[q] = mk<T>(v[q].x - p.m.dtL * dfdeta(p.m, c.x, v[q].x, s0),
+                             v[q].y - p.m.dtL * dfdeta(p.m, c.y, v[q].y, s1));
+            }
+        }
+    }
+
+    fft_stages<M, E, 1>(v, j, p.tw, buf, sync);
+
+    C *dst = (MODE == ROW_STEP && f == 0) ? (p.zg + row * M) : (p.zst + f * p.zfs + row * M);
+    if (valid) {
+#pragma unroll
+        for (int q = 0; q < E; ++q) dst[j + q * TT] = v[q];
+    }
+}
+
+template <typename T, int M, int E, int MODE>
+static cudaError_t launch_row_inst(const RowParams<T> &p, cudaStream_t s)
+{
+    typedef typename V2<T>::type C;
+    constexpr int TT = M / E;
+    const int per_row = TT * p.F;
+    if (per_row > 1024) return cudaErrorInvalidConfiguration;
+    int RB = 256 / per_row;
+    if (RB < 1) RB = 1;
+    if (RB > p.nrows) RB = p.nrows;
+    const int threads = RB * per_row;
+    const size_t smem = (size_t)RB * p.F * row_pitch<M, E>() * sizeof(C);
+    auto kern = row_kernel<T, M, E, MODE>;
+    if (smem > 48 * 1024) {
+        cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        if (e != cudaSuccess) return e;
+    }
+    const unsigned grid = (unsigned)((p.nrows + RB - 1) / RB);
+    kern<<<grid, threads, smem, s>>>(p);
+    return cudaGetLastError();
+}
+
+template <typename T, int M, int E>
+static cudaError_t launch_row_mode(int mode, const RowParams<T> &p, cudaStream_t s)
+{
+    switch (mode) {
+    case ROW_SET:  return launch_row_inst<T, M, E, ROW_SET>(p, s);
+    case ROW_STEP: return launch_row_inst<T, M, E, ROW_STEP>(p, s);
+    case ROW_GET:  return launch_row_inst<T, M, E, ROW_GET>(p, s);
+    }
+    return cudaErrorInvalidValue;
+}
+
+template <typename T> cudaError_t launch_row(int mode, int nx, const RowParams<T> &p, cudaStream_t s)
+{
+    switch (nx / 2) {
+    case 8:    return launch_row_mode<T, 8, 8>(mode, p, s);
+    case 16:   return launch_row_mode<T, 16, 8>(mode, p, s);
+    case 32:   return launch_row_mode<T, 32, 8>(mode, p, s);
+    case 64:   return launch_row_mode<T, 64, 8>(mode, p, s);
+    case 128:  return launch_row_mode<T, 128, 8>(mode, p, s);
+    case 256:  return launch_row_mode<T, 256, 8>(mode, p, s);
+    case 512:  return launch_row_mode<T, 512, 8>(mode, p, s);
+    case 1024: return launch_row_mode<T, 1024, 16>(mode, p, s);
+    }
+    return cudaErrorInvalidValue;
+}
+
+template cudaError_t launch_row<double>(int, int, const RowParams<double> &, cudaStream_t);
+template cudaError_t launch_row<float>(int, int, const RowParams<float> &, cudaStream_t);
+
+}  // namespace pf

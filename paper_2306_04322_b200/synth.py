@@ -81,7 +81,7 @@ def init_b(n, n_eta: int, domain: float | None = None):
         x = (np.arange(nx) * dx[0])[None, :]
         y = (np.arange(ny) * dx[1])[:, None]
         c = _eq4(x, y) + 0.0 * (x + y)
-        eta = np.stack([_eq5(i, x, y) + 0.0 * (x + y) for i in range(1, n_eta + 1)])
+        eta = np.stack([_eq5(i, x, y) + 0.0 * (x + y) for i in range(1, n_eta + 1)]) if n_eta else np.zeros((0, ny, nx))
         return np.ascontiguousarray(c), np.ascontiguousarray(eta), dx
     l = 100.0 if domain is None else float(domain)
     nx, ny, nz = n
@@ -92,7 +92,7 @@ def init_b(n, n_eta: int, domain: float | None = None):
     c = np.full((nz, ny, nx), C0)
     eta = np.stack([0.5 * (1.0 + np.tanh(np.arctan(2.0 * _eq5(i, 2.0 * x, 2.0 * y) - 1.0)
                                          - ((z - l / 2.0) / 5.0) ** 4))
-                    for i in range(1, n_eta + 1)])
+                    for i in range(1, n_eta + 1)]) if n_eta else np.zeros((0, nz, ny, nx))
     return c, np.ascontiguousarray(eta), dx
 
 

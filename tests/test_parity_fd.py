@@ -1,0 +1,63 @@
+"""GPU parity of the explicit finite-difference step (pf_step_fd) and of pf_free_energy against the oracle."""
+import numpy as np
+import pytest
+
+from paper_2306_04322_b200 import pf
+from parity_util import make_init, rel_linf, run_both
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.mark.parametrize("n,n_eta,steps", [((64, 64), 2, 500), ((32, 128), 4, 100), ((16, 32, 64), 2, 100), ((64, 32), 0, 50)])
+def test_fd_parity_fp64(oracle, n, n_eta, steps):
+    # dt = 0.75 x the linear Cahn-Hilliard stability limit of the grid, capped at 2e-3:
+    # init B has dx = l/n (coarse) and eta = O(1), where the Allen-Cahn reaction term limits dt instead
+    c, eta, dx = make_init("B", n, n_eta)
+    kt2 = sum(4.0 / d ** 2 for d in dx)
+    dt = min(0.75 * 2.0 / (5.0 * kt2 * (4.0 + 3.0 * kt2)), 2e-3)
+    (gc, geta), (rc, reta) = run_both(oracle, n=n, n_eta=n_eta, init="B", steps=steps, dt=dt, method="fd")
+    assert rel_linf([gc, geta], [rc, reta]) < 1e-12
+
+
+def test_fd_c1_noise_dx1(oracle):
+    # configs[0] FD leg: dx = 1, dt = 0.75 * 1.786e-3
+    (gc, geta), (rc, reta) = run_both(oracle, n=(64, 64), n_eta=2, init="A", steps=1000, dt=0.75 * 2.0 / (5 * 8 * (4 + 24)), method="fd")
+    assert rel_linf([gc, geta], [rc, reta]) < 1e-12
+
+
+def test_fd_fp32(oracle):
+    (gc, geta), (rc, reta) = run_both(oracle, n=(64, 64), n_eta=2, init="B", steps=200, dt=1e-3, method="fd", precision="f32")
+    assert rel_linf([gc, geta], [rc, reta]) < 1e-4
+
+
+def test_fs_then_fd_then_fs_state_handoff(oracle):
+    n, p = (64, 32), 2
+    c, eta, dx = make_init("B", n, p)
+    m = oracle.Model(n=n, n_eta=p, dx=dx, dt=1e-3)
+    with pf.Context(n, n_eta=p, dx=dx, dt=1e-3) as ctx:
+        ctx.set_fields(c, eta)
+        ctx.step_fs(7); ctx.step_fd(5); ctx.step_fs(3)
+        gc, geta = ctx.get_fields()
+    rc, reta = m.step_fs(c, eta, 7)
+    rc, reta = m.step_fd(rc, reta, 5)
+    rc, reta = m.step_fs(rc, reta, 3)
+    assert rel_linf([gc, geta], [rc, reta]) < 1e-10
+
+
+@pytest.mark.parametrize("n", [(64, 128), (32, 16, 64)])
+@pytest.mark.parametrize("kind", [0, 1])
+def test_free_energy(oracle, n, kind):
+    p = 3
+    c, eta, dx = make_init("B", n, p)
+    m = oracle.Model(n=n, n_eta=p, dx=dx, dt=5e-3)
+    with pf.Context(n, n_eta=p, dx=dx, dt=5e-3) as ctx:
+        ctx.set_fields(c, eta)
+        e0 = ctx.free_energy(kind)
+        ctx.step_fs(10)
+        e1 = ctx.free_energy(kind)
+        gc, geta = ctx.get_fields()
+    np.testing.assert_allclose(e0, m.free_energy(c, eta, kind), rtol=1e-11)
+    rc, reta = m.step_fs(c, eta, 10)
+    np.testing.assert_allclose(e1, m.free_energy(rc, reta, kind), rtol=1e-9)
+    assert e1[0] < e0[0]                      # monotone decrease
+    assert rel_linf([gc, geta], [rc, reta]) < 1e-10
