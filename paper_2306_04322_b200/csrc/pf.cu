@@ -270,7 +270,7 @@ template <typename T> int step_fs(pf_ctx *c, int nsteps)
         for (int k = 0; k < c->nk; ++k) c->kms[k] = sum[k] / nsteps;
     } else {
         // replay one captured step; small grids are launch-latency bound without it
-        if (!c->fs_graph && c->graph_ok && nsteps >= 2) {
+        if (!c->fs_graph && c->graph_ok) {
             cudaGraph_t g = nullptr;
             const long long before = c->launches;
             if (cudaStreamBeginCapture(c->stream, cudaStreamCaptureModeThreadLocal) == cudaSuccess) {
