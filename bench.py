@@ -67,13 +67,13 @@ def bytes_model(n, p, w):
     S = (n[0] // 2 + 1) * (N // n[0]) * 2 * w
     if len(n) == 2:
         survey = F * (2 * R + 7 * S)
-        kern = {"row_c2r_nonlinear_r2c": 2 * F * R, "col_y_update_c": 3 * R, "col_y_update_eta": 2 * p * R}
+        kern = {"row_c2r_nonlinear_r2c": 2 * F * R, "col_y_fft_update_ifft": (3 + 2 * p) * R}
     else:
         survey = F * (2 * R + 11 * S)
         P2 = ((n[0] // 2 + 1 + 15) // 16) * 16
         Sp = P2 * n[1] * n[2] * 2 * w          # one padded half-spectrum array as stored
-        kern = {"row_c2r_nonlinear_r2c": 2 * F * R, "col_y_fwd_g": R + Sp, "col_y_fwd_eta": p * (R + Sp),
-                "col_z_update_c": 3 * Sp, "col_z_update_eta": 2 * p * Sp, "col_y_inv": F * (Sp + R)}
+        kern = {"row_c2r_nonlinear_r2c": 2 * F * R, "col_y_fwd": F * (R + Sp),
+                "col_z_fft_update_ifft": (3 + 2 * p) * Sp, "col_y_inv": F * (Sp + R)}
     return survey, kern
 
 

@@ -25,6 +25,7 @@ namespace {
 
 enum State { ST_NONE = 0, ST_REAL = 1, ST_SPECTRAL = 2, ST_BOTH = 3 };
 const int kMaxFsKernels = 6;
+const int kProfBatch = 16;
 
 }  // namespace
 
@@ -54,7 +55,7 @@ struct pf_ctx {
     int nk = 0;
     const char *kname[kMaxFsKernels] = {};
     double kms[kMaxFsKernels] = {};
-    cudaEvent_t ev[kMaxFsKernels + 1] = {};
+    std::vector<cudaEvent_t> pev;
 };
 
 namespace {
@@ -167,65 +168,66 @@ template <typename T> ColParams<T> col_params(pf_ctx *c)
 }
 
 struct KernelTimer {
-    pf_ctx *c; int k = 0;
-    explicit KernelTimer(pf_ctx *ctx) : c(ctx) { if (c->profiling) cudaEventRecord(c->ev[0], c->stream); }
+    pf_ctx *c; int k = 0; cudaEvent_t *ev;
+    KernelTimer(pf_ctx *ctx, cudaEvent_t *events) : c(ctx), ev(events) { if (ev) cudaEventRecord(ev[0], c->stream); }
     void mark(const char *name)
     {
-        if (k < kMaxFsKernels) { c->kname[k] = name; if (c->profiling) cudaEventRecord(c->ev[k + 1], c->stream); ++k; }
+        if (k < kMaxFsKernels) { c->kname[k] = name; if (ev) cudaEventRecord(ev[k + 1], c->stream); ++k; }
     }
 };
 
-// 3D: (kx,ky)-spectral planes of the listed z-form fields: s2[f] (or g2) <- FFT_y(unpack(z-form))
-template <typename T> cudaError_t mid_forward(pf_ctx *c, const void *zsrc, long zfs, void *dst, long dfs, int nfields)
+// 3D: (kx,ky)-spectral planes of z-form arrays: dst slot s <- FFT_y(unpack(src slot s)); with galt, slot 0 is zg -> g2
+template <typename T> cudaError_t mid_forward(pf_ctx *c, const void *zsrc, long zfs, void *dst, long dfs, int nslots,
+                                              bool galt, bool pdl)
 {
     typedef typename V2<T>::type C;
     const int ny = c->p.n[1], nz = c->p.n[2];
     ColParams<T> q = col_params<T>(c);
     q.in0 = (const C *)zsrc; q.in_fs = zfs; q.in_rs = c->M; q.in_bs = (long)ny * c->M;
     q.out = (C *)dst; q.out_fs = dfs; q.out_rs = c->P2; q.out_bs = (long)ny * c->P2;
+    if (galt) { q.alt_in = (const C *)c->zg; q.alt_out = (C *)c->g2; }
     q.tw = (const C *)c->tw_y;
+    q.pdl = pdl;
     ++c->launches;
-    return launch_col<T>(COL_3D_MIDFWD, false, ny, nfields, nz, q, c->stream);
+    return launch_col<T>(COL_3D_MIDFWD, ny, nslots, nz, q, c->stream);
 }
 
-template <typename T> int fs_one_step(pf_ctx *c)
+// One FS step. 2D: x kernel, y kernel. 3D: x kernel, y-forward, z kernel, y-inverse. All launched with programmatic
+// stream serialization: each kernel's prologue overlaps its predecessor's tail (griddepcontrol in the kernels).
+template <typename T> int fs_one_step(pf_ctx *c, cudaEvent_t *events)
 {
     typedef typename V2<T>::type C;
-    const int ny = c->p.n[1], nz = c->p.n[2], p = c->p.n_eta;
+    const int ny = c->p.n[1], nz = c->p.n[2];
     const long zfs = c->N / 2;
-    KernelTimer kt(c);
+    const bool pdl = events == nullptr;                 // timed launches are kept strictly serial
+    KernelTimer kt(c, events);
     RowParams<T> r = row_params<T>(c);
+    r.pdl = pdl;
     PF_CK(c, launch_row<T>(ROW_STEP, c->p.n[0], r, c->stream)); ++c->launches; kt.mark("row_c2r_nonlinear_r2c");
     C *zst = (C *)c->zst;
     if (c->p.ndim == 2) {
         ColParams<T> q = col_params<T>(c);
         q.tw = (const C *)c->tw_y;
         q.in_rs = q.out_rs = c->M;
-        q.in0 = zst; q.in1 = (const C *)c->zg; q.out = zst;
-        PF_CK(c, launch_col<T>(COL_2D_LAST, true, ny, 1, 1, q, c->stream)); ++c->launches; kt.mark("col_y_update_c");
-        if (p > 0) {
-            q.in0 = zst + zfs; q.out = zst + zfs; q.in_fs = q.out_fs = zfs; q.in1 = nullptr;
-            PF_CK(c, launch_col<T>(COL_2D_LAST, false, ny, p, 1, q, c->stream)); ++c->launches; kt.mark("col_y_update_eta");
-        }
+        q.in0 = zst; q.in1 = (const C *)c->zg; q.out = zst; q.in_fs = q.out_fs = zfs;
+        q.has_c = 1; q.pdl = pdl;
+        PF_CK(c, launch_col<T>(COL_2D_LAST, ny, c->F, 1, q, c->stream)); ++c->launches; kt.mark("col_y_fft_update_ifft");
     } else {
         const long s2fs = (long)nz * ny * c->P2;
         C *s2 = (C *)c->s2;
-        PF_CK(c, mid_forward<T>(c, c->zg, 0, c->g2, 0, 1)); kt.mark("col_y_fwd_g");
-        if (p > 0) { PF_CK(c, mid_forward<T>(c, zst + zfs, zfs, s2 + s2fs, s2fs, p)); kt.mark("col_y_fwd_eta"); }
+        PF_CK(c, mid_forward<T>(c, zst, zfs, s2, s2fs, c->F, true, pdl)); kt.mark("col_y_fwd");
         ColParams<T> q = col_params<T>(c);
         q.tw = (const C *)c->tw_z;
         q.in_rs = q.out_rs = (long)ny * c->P2; q.ncols = ny * c->P2;
-        q.in0 = s2; q.in1 = (const C *)c->g2; q.out = s2;
-        PF_CK(c, launch_col<T>(COL_3D_LAST, true, nz, 1, 1, q, c->stream)); ++c->launches; kt.mark("col_z_update_c");
-        if (p > 0) {
-            q.in0 = s2 + s2fs; q.out = s2 + s2fs; q.in_fs = q.out_fs = s2fs; q.in1 = nullptr;
-            PF_CK(c, launch_col<T>(COL_3D_LAST, false, nz, p, 1, q, c->stream)); ++c->launches; kt.mark("col_z_update_eta");
-        }
+        q.in0 = s2; q.in1 = (const C *)c->g2; q.out = s2; q.in_fs = q.out_fs = s2fs;
+        q.has_c = 1; q.pdl = pdl;
+        PF_CK(c, launch_col<T>(COL_3D_LAST, nz, c->F, 1, q, c->stream)); ++c->launches; kt.mark("col_z_fft_update_ifft");
         ColParams<T> v = col_params<T>(c);
         v.tw = (const C *)c->tw_y;
         v.in0 = s2; v.in_fs = s2fs; v.in_rs = c->P2; v.in_bs = (long)ny * c->P2;
         v.out = zst; v.out_fs = zfs; v.out_rs = c->M; v.out_bs = (long)ny * c->M;
-        PF_CK(c, launch_col<T>(COL_3D_MIDINV, false, ny, c->F, nz, v, c->stream)); ++c->launches; kt.mark("col_y_inv");
+        v.pdl = pdl;
+        PF_CK(c, launch_col<T>(COL_3D_MIDINV, ny, c->F, nz, v, c->stream)); ++c->launches; kt.mark("col_y_inv");
     }
     c->nk = kt.k;
     return PF_OK;
@@ -240,7 +242,7 @@ template <typename T> int to_spectral(pf_ctx *c)
         c->state = ST_BOTH;
     }
     if (c->p.ndim == 3 && !c->s2c_valid) {
-        PF_CK(c, mid_forward<T>(c, c->zst, 0, c->s2, 0, 1));
+        PF_CK(c, mid_forward<T>(c, c->zst, 0, c->s2, 0, 1, false, false));
         c->s2c_valid = true;
     }
     return PF_OK;
@@ -261,11 +263,24 @@ template <typename T> int step_fs(pf_ctx *c, int nsteps)
     int rc = to_spectral<T>(c);
     if (rc) return rc;
     if (c->profiling) {
+        // events around every kernel; a batch of steps is queued before the host waits, so launch latency stays hidden
+        const int B = kProfBatch, per = kMaxFsKernels + 1;
+        if (c->pev.empty()) {
+            c->pev.resize((size_t)B * per);
+            for (auto &e : c->pev) PF_CK(c, cudaEventCreate(&e));
+        }
         double sum[kMaxFsKernels] = {};
-        for (int s = 0; s < nsteps; ++s) {
-            if ((rc = fs_one_step<T>(c))) return rc;
-            PF_CK(c, cudaEventSynchronize(c->ev[c->nk]));
-            for (int k = 0; k < c->nk; ++k) { float ms = 0; cudaEventElapsedTime(&ms, c->ev[k], c->ev[k + 1]); sum[k] += ms; }
+        for (int s0 = 0; s0 < nsteps; s0 += B) {
+            const int nb = (nsteps - s0 < B) ? nsteps - s0 : B;
+            for (int s = 0; s < nb; ++s)
+                if ((rc = fs_one_step<T>(c, c->pev.data() + (size_t)s * per))) return rc;
+            PF_CK(c, cudaStreamSynchronize(c->stream));
+            for (int s = 0; s < nb; ++s)
+                for (int k = 0; k < c->nk; ++k) {
+                    float ms = 0;
+                    cudaEventElapsedTime(&ms, c->pev[(size_t)s * per + k], c->pev[(size_t)s * per + k + 1]);
+                    sum[k] += ms;
+                }
         }
         for (int k = 0; k < c->nk; ++k) c->kms[k] = sum[k] / nsteps;
     } else {
@@ -274,7 +289,7 @@ template <typename T> int step_fs(pf_ctx *c, int nsteps)
             cudaGraph_t g = nullptr;
             const long long before = c->launches;
             if (cudaStreamBeginCapture(c->stream, cudaStreamCaptureModeThreadLocal) == cudaSuccess) {
-                rc = fs_one_step<T>(c);
+                rc = fs_one_step<T>(c, nullptr);
                 cudaError_t e = cudaStreamEndCapture(c->stream, &g);
                 c->fs_graph_nodes = (int)(c->launches - before);
                 c->launches = before;
@@ -290,7 +305,7 @@ template <typename T> int step_fs(pf_ctx *c, int nsteps)
         }
         for (int s = 0; s < nsteps; ++s) {
             if (c->fs_graph) { PF_CK(c, cudaGraphLaunch(c->fs_graph, c->stream)); c->launches += c->fs_graph_nodes; }
-            else if ((rc = fs_one_step<T>(c))) return rc;
+            else if ((rc = fs_one_step<T>(c, nullptr))) return rc;
         }
     }
     c->state = ST_SPECTRAL;
@@ -341,13 +356,13 @@ template <typename T> int free_energy(pf_ctx *c, int kind, double *out)
         const int ny = c->p.n[1], nz = c->p.n[2];
         if (c->p.ndim == 2) {
             q.tw = (const C *)c->tw_y; q.in0 = (const C *)c->zst; q.in_fs = c->N / 2; q.in_rs = c->M;
-            PF_CK(c, launch_col<T>(COL_2D_ENERGY, false, ny, c->F, 1, q, c->stream)); ++c->launches;
+            PF_CK(c, launch_col<T>(COL_2D_ENERGY, ny, c->F, 1, q, c->stream)); ++c->launches;
         } else {
             const long s2fs = (long)nz * ny * c->P2;
-            if (p > 0) PF_CK(c, mid_forward<T>(c, (C *)c->zst + c->N / 2, c->N / 2, (C *)c->s2 + s2fs, s2fs, p));
+            if (p > 0) PF_CK(c, mid_forward<T>(c, (C *)c->zst + c->N / 2, c->N / 2, (C *)c->s2 + s2fs, s2fs, p, false, false));
             q.tw = (const C *)c->tw_z; q.in0 = (const C *)c->s2; q.in_fs = s2fs; q.in_rs = (long)ny * c->P2;
             q.ncols = ny * c->P2;
-            PF_CK(c, launch_col<T>(COL_3D_ENERGY, false, nz, c->F, 1, q, c->stream)); ++c->launches;
+            PF_CK(c, launch_col<T>(COL_3D_ENERGY, nz, c->F, 1, q, c->stream)); ++c->launches;
         }
         scale_grad = 1.0 / (double)c->N;
     }
@@ -396,7 +411,7 @@ void pf_destroy(pf_ctx *c)
 {
     if (!c) return;
     drop_graph(c);
-    for (auto &e : c->ev) if (e) cudaEventDestroy(e);
+    for (auto &e : c->pev) if (e) cudaEventDestroy(e);
     void *bufs[] = {c->real[0], c->real[1], c->zst, c->zg, c->s2, c->g2, c->mu, c->tw_m, c->tw_y, c->tw_z,
                     c->tw_nx, c->kx2, c->ky2, c->kz2, c->acc};
     for (void *b : bufs) if (b) cudaFree(b);
@@ -454,7 +469,6 @@ int pf_create(const pf_params *p, pf_ctx **out)
     }
     rc = (p->precision == PF_F64) ? upload_tables<double>(c) : upload_tables<float>(c);
     if (rc) return fail(rc);
-    for (auto &e : c->ev) if (cudaEventCreate(&e) != cudaSuccess) return fail(PF_ECUDA);
     *out = c;
     return PF_OK;
 }
@@ -532,8 +546,7 @@ int pf_set_profiling(pf_ctx *c, int on)
 int pf_num_fs_kernels(const pf_ctx *c)
 {
     if (!c) return 0;
-    const int e = c->p.n_eta > 0 ? 1 : 0;
-    return c->p.ndim == 2 ? 2 + e : 4 + 2 * e;
+    return c->p.ndim == 2 ? 2 : 4;
 }
 double pf_fs_kernel_ms(pf_ctx *c, int which) { return (c && which >= 0 && which < c->nk) ? c->kms[which] : -1.0; }
 const char *pf_fs_kernel_name(const pf_ctx *c, int which) { return (c && which >= 0 && which < c->nk && c->kname[which]) ? c->kname[which] : ""; }

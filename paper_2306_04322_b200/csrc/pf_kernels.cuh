@@ -29,6 +29,7 @@ template <typename T> struct RowParams {
     long     rfs;            // field stride of real in reals (= nrows*nx)
     int      nrows;          // ny*nz
     int      F;              // 1 + n_eta
+    int      pdl;            // launch with programmatic stream serialization
     Model<T> m;
 };
 
@@ -44,10 +45,14 @@ enum ColMode {
 
 template <typename T> struct ColParams {
     typedef typename V2<T>::type C;
-    const C *in0;            // primary input  (eta fields: w = eta - dt L h; c field: the state u)
-    const C *in1;            // c field only: g = df/dc
-    C       *out;
-    long     in_fs, in1_fs, out_fs;   // field strides (blockIdx.z)
+    const C *in0;            // input of slot s: in0 + s*in_fs  (eta fields: w = eta - dt L h; slot 0: the c state)
+    const C *in1;            // update modes with has_c: g = df/dc (same layout as slot 0 of in0)
+    C       *out;            // output of slot s: out + s*out_fs
+    const C *alt_in;         // if non-null, slot 0 reads alt_in and writes alt_out instead (3D y-forward of g)
+    C       *alt_out;
+    int      has_c;          // update modes: slot 0 is the Cahn-Hilliard field (needs in1)
+    int      pdl;            // launch with programmatic stream serialization
+    long     in_fs, out_fs;  // slot strides (blockIdx.z)
     long     in_bs, out_bs;           // batch strides (blockIdx.y; 3D mid kernels: z planes)
     long     in_rs, out_rs;           // stride between consecutive elements along the FFT axis
     int      M;              // nx/2
@@ -59,6 +64,7 @@ template <typename T> struct ColParams {
     const T *ky2;            // per ky (2D last: the FFT axis; 3D last: the middle axis)
     const T *kz2;            // per kz (3D last: the FFT axis)
     double  *acc;            // energy modes: accumulator (one double per field)
+    int      bar_off;        // byte offset of the mbarriers in dynamic shared memory (set by the launcher)
     Model<T> m;
 };
 
@@ -85,11 +91,30 @@ template <typename T> struct EnergyParams {
 
 // ---- launchers (defined in the .cu files; return cudaGetLastError()) ----
 template <typename T> cudaError_t launch_row(int mode, int nx, const RowParams<T> &p, cudaStream_t s);
-template <typename T> cudaError_t launch_col(int mode, bool is_c, int nfft, int nfields, int nbatch,
-                                             const ColParams<T> &p, cudaStream_t s);
+template <typename T> cudaError_t launch_col(int mode, int nfft, int nslots, int nbatch, const ColParams<T> &p, cudaStream_t s);
 template <typename T> cudaError_t launch_fd_mu(const FdParams<T> &p, cudaStream_t s);
 template <typename T> cudaError_t launch_fd_update(const FdParams<T> &p, cudaStream_t s);
 template <typename T> cudaError_t launch_energy(const EnergyParams<T> &p, cudaStream_t s);
+
+#if defined(__CUDACC__)
+// Programmatic dependent launch: a kernel launched with the attribute may start while its predecessor in the
+// stream is still running; it must not touch data the predecessor produces (or still reads) before
+// grid_dependency_wait(), which returns once the predecessor grid has completed and flushed.
+__device__ __forceinline__ void grid_dependency_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
+__device__ __forceinline__ void grid_dependents_launch() { asm volatile("griddepcontrol.launch_dependents;" ::: "memory"); }
+
+template <typename K, typename P>
+static inline cudaError_t launch_pdl(K kern, dim3 grid, dim3 block, size_t smem, cudaStream_t s, bool pdl, const P &params)
+{
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = grid; cfg.blockDim = block; cfg.dynamicSmemBytes = smem; cfg.stream = s;
+    cudaLaunchAttribute at[1];
+    at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    at[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = at; cfg.numAttrs = pdl ? 1 : 0;
+    return cudaLaunchKernelEx(&cfg, kern, params);
+}
+#endif
 
 // pointwise model, shared by the row kernel, the FD kernels and the energy kernel --------------------
 // h(eta) = sum eta^3 (6 eta^2 - 15 eta + 10); g(eta) = sum eta^2 (1-eta)^2 + alpha sum_i sum_{j!=i} eta_i^2 eta_j^2

@@ -30,9 +30,15 @@ struct CtaSync { __device__ __forceinline__ void operator()() const { __syncthre
 
 template <int M, int E> __host__ __device__ constexpr int row_pitch() { return M + (M >> 3) + 1; }
 
+// Register cap: the kernel is bound by fp64 issue and shared-memory exchange latency, so resident warps matter more
+// than the last few registers (measured on B200: 94 -> 80 registers: 1024^2 row kernel 28.1 -> 26.4 us; 64 at
+// nx = 256: 394 -> 317 us at 256^3).
 template <typename T, int M, int E, int MODE>
-__global__ void row_kernel(const RowParams<T> p)
+__global__ void __maxnreg__((M >= 256) ? 80 : 64) row_kernel(const RowParams<T> p)
 {
+#ifdef PF_DBG_EMPTY
+    return;
+#endif
     typedef typename V2<T>::type C;
     constexpr int TT = M / E;
     constexpr int MP = row_pitch<M, E>();
@@ -50,6 +56,9 @@ __global__ void row_kernel(const RowParams<T> p)
     const bool valid = row < p.nrows;
     RowBuf<C, 3> buf{smem + (long)rf * MP};
     CtaSync sync;
+
+    grid_dependency_wait();
+    grid_dependents_launch();
 
     C v[E];
     if (MODE == ROW_SET) {
@@ -86,15 +95,19 @@ __global__ void row_kernel(const RowParams<T> p)
         for (int q = 0; q < E; ++q) {
             const int n = j + q * TT;
             const int np = n + (n >> 3);
-            T h0 = 0, h1 = 0, s0 = 0, s1 = 0;
-            for (int ff = 1; ff < F; ++ff) {
-                const C e = rowbase[(long)ff * MP + np];
-                h0 += h_term(e.x); h1 += h_term(e.y);
-                s0 += e.x * e.x;   s1 += e.y * e.y;
-            }
             if (f == 0) {
+                T h0 = 0, h1 = 0;                        // h(eta) = sum_i eta_i^3 (6 eta_i^2 - 15 eta_i + 10)
+                for (int ff = 1; ff < F; ++ff) {
+                    const C e = rowbase[(long)ff * MP + np];
+                    h0 += h_term(e.x); h1 += h_term(e.y);
+                }
                 v[q] = mk<T>(dfdc(p.m, v[q].x, h0), dfdc(p.m, v[q].y, h1));
             } else {
+                T s0 = 0, s1 = 0;                        // sum_j eta_j^2 (own field included)
+                for (int ff = 1; ff < F; ++ff) {
+                    const C e = rowbase[(long)ff * MP + np];
+                    s0 += e.x * e.x; s1 += e.y * e.y;
+                }
                 const C c = rowbase[np];
                 v[q] = mk<T>(v[q].x - p.m.dtL * dfdeta(p.m, c.x, v[q].x, s0),
                              v[q].y - p.m.dtL * dfdeta(p.m, c.y, v[q].y, s1));
@@ -129,8 +142,7 @@ static cudaError_t launch_row_inst(const RowParams<T> &p, cudaStream_t s)
         if (e != cudaSuccess) return e;
     }
     const unsigned grid = (unsigned)((p.nrows + RB - 1) / RB);
-    kern<<<grid, threads, smem, s>>>(p);
-    return cudaGetLastError();
+    return launch_pdl(kern, dim3(grid), dim3(threads), smem, s, p.pdl != 0, p);
 }
 
 template <typename T, int M, int E>

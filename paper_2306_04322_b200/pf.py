@@ -13,7 +13,7 @@ import os
 import numpy as np
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
-SO_PATH = os.path.join(_HERE, "libpf.so")
+SO_PATH = os.environ.get("PF_LIBPF") or os.path.join(_HERE, "libpf.so")      # PF_LIBPF: explicit path override
 
 PF_F32, PF_F64 = 0, 1
 PF_HOST, PF_DEVICE = 0, 1
