@@ -149,10 +149,60 @@ def run_reference(args):
     print(json.dumps(line), flush=True)
 
 
+def cufft_side_reference(torch, n, p, prec, dx, dt, c0, eta0, stream, steps=20):
+    """Side reference only (north_star): the same FS step assembled from cuFFT (torch.fft.rfftn/irfftn) and elementwise
+    torch ops, timed in the same process. Not part of the product path and not compared for parity here."""
+    dev = torch.device("cuda")
+    tdt = torch.float64 if prec == "f64" else torch.float32
+    M_, L_, kc, ke, rho2, ca, cb, w_, al = 5.0, 5.0, 3.0, 3.0, 2.0, 0.3, 0.7, 1.0, 5.0
+    nd = len(n)
+    with torch.cuda.stream(stream):
+        c = torch.as_tensor(c0, dtype=tdt, device=dev)
+        eta = torch.as_tensor(eta0, dtype=tdt, device=dev)
+        k2 = None
+        for d in range(nd):                       # array axis nd-1-d has length n[d] (x fastest)
+            ax = nd - 1 - d
+            freq = torch.fft.rfftfreq(n[d], d=dx[d]) if ax == nd - 1 else torch.fft.fftfreq(n[d], d=dx[d])
+            kk = (2 * np.pi * freq.to(tdt).to(dev)) ** 2
+            shape = [1] * nd
+            shape[ax] = kk.numel()
+            k2 = kk.reshape(shape) if k2 is None else k2 + kk.reshape(shape)
+        dc = 1.0 / (1.0 + dt * M_ * kc * k2 * k2)
+        de = 1.0 / (1.0 + dt * L_ * ke * k2)
+        ch = torch.fft.rfftn(c)
+        eh = torch.fft.rfftn(eta, dim=tuple(range(1, nd + 1)))
+        dims = tuple(range(-nd, 0))
+
+        def step(ch, eh):
+            c = torch.fft.irfftn(ch, s=c0.shape, dim=dims)
+            eta = torch.fft.irfftn(eh, s=c0.shape, dim=dims)
+            h = (eta ** 3 * (6 * eta ** 2 - 15 * eta + 10)).sum(0)
+            s2 = (eta ** 2).sum(0)
+            g = 2 * rho2 * ((c - ca) * (1 - h) - (cb - c) * h)
+            fba = rho2 * ((cb - c) ** 2 - (c - ca) ** 2)
+            hh = fba * 30 * eta ** 2 * (1 - eta) ** 2 + w_ * (2 * eta * (1 - eta) * (1 - 2 * eta) + 4 * al * eta * (s2 - eta ** 2))
+            gh = torch.fft.rfftn(g, dim=dims)
+            hh = torch.fft.rfftn(hh, dim=dims)
+            return (ch - dt * M_ * k2 * gh) * dc, (eh - dt * L_ * hh) * de
+
+        for _ in range(3):
+            ch, eh = step(ch, eh)
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        torch.cuda.synchronize()
+        e0.record(stream)
+        for _ in range(steps):
+            ch, eh = step(ch, eh)
+        e1.record(stream)
+        torch.cuda.synchronize()
+    ms = e0.elapsed_time(e1) / steps
+    return {"value": 1e3 / ms, "unit": "steps/s", "ms_per_step": ms, "steps": steps,
+            "what": "torch.fft.rfftn/irfftn (cuFFT) + elementwise torch ops, single simulation, same workload"}
+
+
 def run_ours(args):
     import torch
     import torch.distributed as dist
-    from paper_2306_04322_b200 import pf
+    from paper_2306_04322_b200 import pf, replicas
 
     rank = int(os.environ.get("RANK", "0"))
     world = int(os.environ.get("WORLD_SIZE", "1"))
@@ -175,7 +225,7 @@ def run_ours(args):
     stream = torch.cuda.Stream()
     ctxs = [pf.Context(n, n_eta=p, dx=dx, dt=dt, precision=prec, stream=stream.cuda_stream) for _ in range(reps)]
     for i, cx in enumerate(ctxs):
-        cx.set_fields(c0 + 1e-4 * i, eta0)
+        cx.set_fields(replicas.perturb(c0, rank, i, reps), eta0)
     torch.cuda.synchronize()
 
     def barrier():
@@ -195,12 +245,7 @@ def run_ours(args):
         run_steps(k, which)
         e1.record(stream)
         barrier()
-        ms = e0.elapsed_time(e1)
-        if world > 1:
-            t = torch.tensor([ms], device="cuda", dtype=torch.float64)
-            dist.all_reduce(t, op=dist.ReduceOp.MAX)
-            ms = float(t.item())
-        return ms
+        return replicas.max_over_ranks(e0.elapsed_time(e1), device="cuda")
 
     K, W = args.steps, max(args.warmup, 3)
     run_steps(W * len(ctxs), ctxs)
@@ -209,11 +254,11 @@ def run_ours(args):
     ms = timed(K, ctxs)
     launches = sum(cx.launch_count() for cx in ctxs) - l0
     clocks = sampler.stop() if sampler else {}
-    value = world * K / (ms * 1e-3)
+    value = replicas.job_throughput(K, ms, world)
 
     # single simulation, state resident in L2 where it fits (reported, not the headline)
     ms_res = timed(K, ctxs[:1])
-    resident = world * K / (ms_res * 1e-3)
+    resident = replicas.job_throughput(K, ms_res, world)
 
     # per-kernel device times (CUDA events on the context's stream, library-side), same cycling as the timed region
     for cx in ctxs:
@@ -264,10 +309,7 @@ def run_ours(args):
         e2e_step()
     torch.cuda.synchronize()
     e2e_s = time.perf_counter() - t0
-    if world > 1:
-        t = torch.tensor([e2e_s], device="cuda", dtype=torch.float64)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        e2e_s = float(t.item())
+    e2e_s = replicas.max_over_ranks(e2e_s, device="cuda")
     e2e = {"value": world * ke / e2e_s, "unit": "steps/s", "h2d_bytes_per_step": F * R, "d2h_bytes_per_step": F * R,
            "steps": ke, "note": "pf_set_fields(HOST) + pf_step_fs(1) + pf_get_fields(HOST) per step, pinned host buffers"}
 
@@ -282,6 +324,9 @@ def run_ours(args):
             "field_point_updates_per_s_G": value * N * F / 1e9,
             "l2_resident_single_simulation": {"value": resident, "unit": "steps/s", "gpoint_updates_per_s": resident * N / 1e9},
             "roofline": roofline, "step_roofline": step_roofline, "e2e": e2e, "gpu_launches": int(launches), "clocks": clocks}
+
+    if rank == 0 and not args.no_cufft:
+        line["cufft_side_reference"] = cufft_side_reference(torch, n, p, prec, dx, dt, c0, eta0, stream)
 
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
         from oracle import pfo
@@ -314,6 +359,7 @@ def main():
     ap.add_argument("--workload", default="1024sq", choices=sorted(WORKLOADS))
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-cufft", action="store_true", help="skip the cuFFT side reference")
     args = ap.parse_args()
     if args.steps is None:
         args.steps = DEFAULT_STEPS[args.workload] if args.impl == "ours" else 20
