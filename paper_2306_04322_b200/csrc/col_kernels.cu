@@ -1,69 +1,100 @@
 // col_kernels.cu -- strided-direction kernels of the Fourier-spectral step.
 //
-// A CTA is two independent thread GROUPS; a group owns TP "units" of two columns each and all N elements of
-// them along the FFT axis; thread (t, j) of a group holds elements j + q*TT of both columns of unit t in
-// registers (fft_core.cuh) and the two transforms run half a stage out of phase (fft2_pipelined).
-// Consecutive lanes map to consecutive columns, so every global access of a warp is made of contiguous
-// 16*TP-byte (fp64) pieces, and the strided "transpose" happens in registers + one shared-memory exchange
-// per FFT stage boundary. Groups synchronise only through their own mbarriers, so the two groups of a CTA
-// (and the CTAs of an SM) drift apart and overlap each other's memory, shared-memory and fp64 phases.
+// A CTA is two independent thread GROUPS; a group owns SLOTS = 2*TP adjacent columns and all N elements of each
+// along the FFT axis. Thread (slot, j) of a group holds elements j + q*TT (q < E, TT = N/E) of ONE column in
+// registers (fft_core.cuh), before and after every transform, so the pointwise work is register local. The slot
+// is the fastest thread index: consecutive lanes own consecutive columns, every global access of a warp is made
+// of contiguous 16*SLOTS-byte (fp64) pieces, and the strided "transpose" happens in registers plus one
+// shared-memory exchange per FFT stage boundary (col_buf.cuh). A group synchronises on its own named barrier, so
+// the groups of a CTA and the CTAs of an SM drift apart and overlap each other's memory, shared-memory and fp64
+// phases; one column per thread keeps the kernel at 64 registers, i.e. 32 resident warps per SM.
 //
-// Units in the pair modes are the mirror pairs (k, M-k) of the z-form (row_kernels.cu): with
-//   E = (Z_k + conj Z_{M-k})/2,  O = -(i/2)(Z_k - conj Z_{M-k}),  W = exp(-2 pi i k / nx)
-// the true half-spectrum columns are  U_k = E + W O  and  U_{M-k} = conj(E - W O), pointwise along the
-// column; k = 0 yields the DC and Nyquist columns from Z_0 alone and k = M/2 is its own mirror. The
-// inverse relations repack two updated columns into z-form. The spectral update itself is
+// In the pair modes the columns of a group are TP mirror pairs (u, M-u) of the z-form (row_kernels.cu): with
+//   E = (Z_u + conj Z_{M-u})/2,  O = -(i/2)(Z_u - conj Z_{M-u}),  W = exp(-2 pi i u / nx)
+// the true half-spectrum columns are  U_u = E + W O  (side 0) and  U_{M-u} = conj(E - W O)  (side 1), pointwise
+// along the column; u = 0 yields the DC and Nyquist columns from Z_0 alone and u = M/2 is its own mirror. Both
+// threads of a pair read both z columns (the second read hits L1); after the inverse transform they exchange
+// their results with one warp shuffle and each writes its own z column. The spectral update itself is
 //   c^   <- ( c^ - dt M |xi|^2 g^ ) / ( 1 + dt M kappa_c |xi|^4 )        Eqs. 12, 14
 //   eta^ <- w^ / ( 1 + dt L kappa_eta |xi|^2 ),  w = eta - dt L h        Eqs. 13, 15
 // with |xi|^2 = kx2 + ky2 (+ kz2) from 1-D tables (Eq. 16/19 or the FS-FD variants).
 //
-// Field slots (blockIdx.z): in the update modes slot 0 is c, whose CTA uses its two groups for the two arrays
-// the update needs on the SAME units: group 0 transforms g = df/dc, scales it by dt M |xi|^2 and hands it over
-// through shared memory; group 1 transforms c^, combines, inverts and stores. Every other CTA uses its two
-// groups for two consecutive blocks of units of one array.
+// Field slots (blockIdx.z): in the update modes slot 0 is c, whose CTA uses its two groups for the two arrays the
+// update needs on the SAME columns: group 0 transforms g = df/dc, scales it by dt M |xi|^2 and hands it over
+// through shared memory; group 1 transforms c^, combines, inverts and stores. Every other CTA uses its two groups
+// for two consecutive blocks of columns of one array.
 #include "pf_kernels.cuh"
+#include "col_buf.cuh"
 
 namespace pf {
-
-// Exchange buffer of a group: N rows (index along the FFT axis) x 2*TP column slots (slot = side*TP + t) of one
-// complex each. A quarter warp (8 lanes x 16 B, one shared-memory wavefront when conflict free) covers 8/TP
-// different rows; which rows depends on the access: consecutive rows for the loads (j + q*TT) and for the stores
-// of later stages, rows R apart for the stores of the first stage. The placement below XORs the position of a
-// row's slots inside its 128-byte line with parities of the row index taken over the bit sets
-// {b, b+LR, b+2LR, ..} (LR = log2 of the first-stage radix), which flip under either pattern.
-template <typename C, int TP, int LR> struct ColBuf {
-    C *base;          // buffer start
-    int side, t;      // this thread's column slot
-    __device__ __forceinline__ static int par(int row, int b)
-    {
-        unsigned m = 0;
-#pragma unroll
-        for (int k = b; k < 12; k += LR) m |= 1u << k;
-        return __popc((unsigned)row & m) & 1;
-    }
-    __device__ __forceinline__ int idx(int row) const
-    {
-        if (TP == 4) return row * 8 + ((side ^ par(row, 0)) * 4 + t);                            // line = 1 row
-        if (TP == 2) return (row >> 1) * 8 + (2 * par(row, 0) + (side ^ par(row, 1))) * 2 + t;   // line = 2 rows
-        return row * (2 * TP) + side * TP + t;
-    }
-    __device__ __forceinline__ void st(int i, C v) { base[idx(i)] = v; }
-    __device__ __forceinline__ C ld(int i) const { return base[idx(i)]; }
-};
 
 __device__ __forceinline__ double rcp(double x) { return __drcp_rn(x); }
 __device__ __forceinline__ float rcp(float x) { return __frcp_rn(x); }
 
+__device__ __forceinline__ double2 shfl_xor1(double2 v)
+{
+    return make_double2(__shfl_xor_sync(0xffffffffu, v.x, 1), __shfl_xor_sync(0xffffffffu, v.y, 1));
+}
+__device__ __forceinline__ float2 shfl_xor1(float2 v)
+{
+    return make_float2(__shfl_xor_sync(0xffffffffu, v.x, 1), __shfl_xor_sync(0xffffffffu, v.y, 1));
+}
+
+// named barrier over the threads of one group (id 0 is __syncthreads)
+struct GroupSync {
+    int id, n;
+    __device__ __forceinline__ void operator()() const { asm volatile("bar.sync %0, %1;" ::"r"(id), "r"(n) : "memory"); }
+};
+
+// Forward transform of the column a thread shares with the TT-1 other threads of its slot. w1 = twiddles of the
+// stage that starts at NS; those of the next stage are requested between the two barriers of the exchange, when
+// the data registers are dead and the table latency hides behind the barrier.
+template <int N, int E, int NS, typename C, typename Buf>
+__device__ __forceinline__ void col_fft(C (&v)[E], int j, const C *__restrict__ tw, Buf &buf, const GroupSync &sync,
+                                        const C (&w1)[StageShape<N, E, NS>::S])
+{
+    stage_compute_w<N, E, NS>(v, w1);
+    constexpr int R = stage_radix(N, E, NS);
+    if constexpr (NS * R < N) {
+        C w2[StageShape<N, E, NS * R>::S];
+        sync();                                   // every thread has taken its elements of the previous exchange
+#ifndef PF_DBG_SKIP_EXCHANGE
+        buf.template store<N, E, NS>(v, j);
+#endif
+        stage_twiddles<N, E, NS * R>(w2, j, tw);
+        sync();
+#ifndef PF_DBG_SKIP_EXCHANGE
+        buf.template load<N, E>(v, j);
+#endif
+        col_fft<N, E, NS * R>(v, j, tw, buf, sync, w2);
+    }
+}
+template <int N, int E, typename C, typename Buf>
+__device__ __forceinline__ void col_fft_forward(C (&v)[E], int j, const C *__restrict__ tw, Buf &buf, const GroupSync &sync)
+{
+    C w0[StageShape<N, E, 1>::S];                 // first stage has no twiddles
+    col_fft<N, E, 1>(v, j, tw, buf, sync, w0);
+}
+
+template <int N, int E, int TP> struct ColShape {
+    static constexpr int TT = N / E;
+    static constexpr int SLOTS = 2 * TP;
+    static constexpr int GT = SLOTS * TT;                               // threads per group (whole warps)
+    static constexpr int THREADS = 2 * GT;
+    static constexpr int MINB = (THREADS >= 1024) ? 1 : 1024 / THREADS;  // 64 registers per thread
+    static constexpr int LR = (E >= 16) ? 4 : 3;                         // log2 of the first-stage radix
+};
+
 template <typename T, int N, int E, int TP, int MODE>
-__global__ void __launch_bounds__(2 * TP *(N / E), (2 * TP * (N / E) >= 512) ? 1 : 512 / (2 * TP * (N / E)))
+__global__ void __launch_bounds__(ColShape<N, E, TP>::THREADS, ColShape<N, E, TP>::MINB)
 col_kernel(const ColParams<T> p)
 {
 #ifdef PF_DBG_EMPTY
     return;
 #endif
     typedef typename V2<T>::type C;
-    constexpr int TT = N / E;
-    constexpr int GT = TP * TT;                        // threads per group (a multiple of 32)
+    typedef ColShape<N, E, TP> Sh;
+    constexpr int TT = Sh::TT, SLOTS = Sh::SLOTS, GT = Sh::GT;
     constexpr bool PAIRS = (MODE == COL_2D_LAST || MODE == COL_3D_MIDFWD || MODE == COL_3D_MIDINV || MODE == COL_2D_ENERGY);
     constexpr bool PAIR_IN = (MODE == COL_2D_LAST || MODE == COL_3D_MIDFWD || MODE == COL_2D_ENERGY);
     constexpr bool PAIR_OUT = (MODE == COL_2D_LAST || MODE == COL_3D_MIDINV);
@@ -72,60 +103,50 @@ col_kernel(const ColParams<T> p)
     constexpr bool DO_UPD = (MODE == COL_2D_LAST || MODE == COL_3D_LAST);
     constexpr bool DO_INV = (MODE == COL_2D_LAST || MODE == COL_3D_LAST || MODE == COL_3D_MIDINV);
     constexpr bool LAST3D = (MODE == COL_3D_LAST || MODE == COL_3D_ENERGY);
-    constexpr int SLOTS = 2 * TP;
-    constexpr int LR = (E >= 16) ? 4 : 3;
     static_assert(GT % 32 == 0, "a group must be whole warps");
 
     extern __shared__ __align__(16) unsigned char smem_raw[];
     const int g = threadIdx.x / GT;                    // group
     const int tg = threadIdx.x - g * GT;
-    const int t = tg % TP;
-    const int j = tg / TP;
+    const int sl = tg % SLOTS;                         // column slot: side = sl & 1, unit t = sl >> 1
+    const int side = sl & 1;
+    const int j = tg / SLOTS;
     const int M = p.M;
-    const int slot = blockIdx.z;
+    const int slot = blockIdx.z;                       // field slot
     const long bz = blockIdx.y;
     const bool c_cta = DO_UPD && p.has_c && slot == 0;
 
-    C *xbuf = reinterpret_cast<C *>(smem_raw) + (long)g * N * SLOTS;
-    PipeBars bars;
-    bars.init(smem_raw + p.bar_off + 32 * g, GT / 32, tg == 0);
-    __syncthreads();
+    ColBuf<C, SLOTS, Sh::LR> buf{reinterpret_cast<C *>(smem_raw) + (long)g * N * SLOTS, sl};
+    const GroupSync sync{1 + g, GT};
 
-    // ---- which block of units, which two columns ----
+    // ---- which block of columns, which column ----
     const int nblk = PAIRS ? (M / 2 + TP) / TP : p.ncols / SLOTS;
     const int ub = c_cta ? (int)blockIdx.x : 2 * (int)blockIdx.x + g;
     bool valid = ub < nblk;
-    bool storeB;
-    int zcolA = 0, zcolB = 0;             // column indices in z-form arrays (pitch M)
-    int pcolA, pcolB;                     // column indices in plain arrays
-    int kxA, kxB;                         // kx of the two columns
-    T base2A, base2B;                     // |xi|^2 contributions that are constant along the column
+    bool store_ok;                        // this thread writes its column
+    int zcolA = 0, zcolB = 0;             // z-form columns of the pair (pitch M)
+    int pcol = 0;                         // column index in plain arrays (half-spectrum planes)
+    int kx;                               // kx of this thread's true spectral column
+    T base2;                              // |xi|^2 contributions that are constant along the column
     C wx = mk<T>(1, 0);                   // exp(-2 pi i u / nx)
     if (PAIRS) {
-        int u = ub * TP + t;
+        int u = ub * TP + (sl >> 1);
         valid = valid && (u <= M / 2);
         if (!valid) u = 0;
         zcolA = u; zcolB = (M - u) & (M - 1);
-        kxA = u; kxB = M - u;
-        pcolA = kxA; pcolB = kxB;
-        storeB = valid && (kxB != kxA);
+        kx = side ? M - u : u;
+        pcol = kx;
+        store_ok = valid && (side == 0 || (PAIR_OUT ? zcolB != zcolA : kx != u));
         wx = p.twx[u];
-        base2A = p.kx2[kxA]; base2B = p.kx2[kxB];
+        base2 = p.kx2[kx];
     } else {
-        pcolA = (valid ? ub : 0) * SLOTS + t; pcolB = pcolA + TP;
-        storeB = valid;
-        kxA = pcolA % p.P2; kxB = pcolB % p.P2;
-        base2A = p.kx2[kxA] + p.ky2[pcolA / p.P2];
-        base2B = p.kx2[kxB] + p.ky2[pcolB / p.P2];
+        pcol = (valid ? ub : 0) * SLOTS + sl;
+        store_ok = valid;
+        kx = pcol % p.P2;
+        base2 = p.kx2[kx] + p.ky2[pcol / p.P2];
     }
-    // a CTA whose two groups both have no units leaves (eta slots are launched with the c slot's grid)
+    // a CTA whose two groups both have no columns leaves (eta slots are launched with the c slot's grid)
     if (!ENERGY && __syncthreads_or(valid) == 0) return;
-    const T *klast = LAST3D ? p.kz2 : p.ky2;
-    T kl[E];
-    if (DO_UPD || ENERGY) {
-#pragma unroll
-        for (int q = 0; q < E; ++q) kl[q] = klast[j + q * TT];       // constant tables: issued early
-    }
 
     // ---- arrays of this CTA / group ----
     const C *in;
@@ -142,8 +163,7 @@ col_kernel(const ColParams<T> p)
     in += bz * p.in_bs;
     out += bz * p.out_bs;
 
-    ColBuf<C, TP, LR> bufA{xbuf, 0, t}, bufB{xbuf, 1, t};
-    C va[E], vb[E];
+    C v[E];
 
     grid_dependency_wait();                // everything above touches constant tables only
     grid_dependents_launch();
@@ -157,20 +177,16 @@ col_kernel(const ColParams<T> p)
             const C e = mk<T>(T(0.5) * (za.x + zb.x), T(0.5) * (za.y - zb.y));
             const C o = mk<T>(T(0.5) * (za.y + zb.y), T(-0.5) * (za.x - zb.x));
             const C wo = cmul(wx, o);
-            va[q] = cadd(e, wo);
-            vb[q] = cconj(csub(e, wo));
+            v[q] = side ? cconj(csub(e, wo)) : cadd(e, wo);
         }
     } else {
 #pragma unroll
-        for (int q = 0; q < E; ++q) {
-            const long i = j + q * TT;
-            va[q] = in[i * p.in_rs + pcolA];
-            vb[q] = in[i * p.in_rs + pcolB];
-        }
+        for (int q = 0; q < E; ++q) v[q] = in[(long)(j + q * TT) * p.in_rs + pcol];
     }
 
-    if (DO_FWD) fft2_pipelined<N, E, 1, true>(va, vb, j, p.tw, bufA, bufB, bars);
+    if (DO_FWD) col_fft_forward<N, E>(v, j, p.tw, buf, sync);
 
+    const T *klast = LAST3D ? p.kz2 : p.ky2;
 #ifndef PF_DBG_SKIP_UPDATE
     if (DO_UPD) {
         const T s = T(1) / T(N);
@@ -178,31 +194,24 @@ col_kernel(const ColParams<T> p)
             // group 0: dt M |xi|^2 g^ -> shared memory (thread-linear in its own buffer) -> group 1
             C *hand = reinterpret_cast<C *>(smem_raw);
             if (g == 0) {
-                asm volatile("bar.sync 1, %0;" ::"r"(GT) : "memory");       // group 0 has left its exchange buffer
+                sync();                                              // group 0 has left its exchange buffer
 #pragma unroll
-                for (int q = 0; q < E; ++q) {
-                    const T ma = p.m.dtM * (base2A + kl[q]), mb = p.m.dtM * (base2B + kl[q]);
-                    hand[(q * 2 + 0) * GT + tg] = cscale(va[q], ma);
-                    hand[(q * 2 + 1) * GT + tg] = cscale(vb[q], mb);
-                }
+                for (int q = 0; q < E; ++q) hand[q * GT + tg] = cscale(v[q], p.m.dtM * (base2 + klast[j + q * TT]));
             }
             __syncthreads();
             if (g == 0) return;
 #pragma unroll
             for (int q = 0; q < E; ++q) {
-                const T k2a = base2A + kl[q], k2b = base2B + kl[q];
-                const T da = s * rcp(T(1) + p.m.dtMkc * k2a * k2a), db = s * rcp(T(1) + p.m.dtMkc * k2b * k2b);
-                const C ga = hand[(q * 2 + 0) * GT + tg], gb = hand[(q * 2 + 1) * GT + tg];
-                va[q] = mk<T>((va[q].x - ga.x) * da, (va[q].y - ga.y) * da);
-                vb[q] = mk<T>((vb[q].x - gb.x) * db, (vb[q].y - gb.y) * db);
+                const T k2 = base2 + klast[j + q * TT];
+                const T d = s * rcp(T(1) + p.m.dtMkc * k2 * k2);
+                const C gq = hand[q * GT + tg];
+                v[q] = mk<T>((v[q].x - gq.x) * d, (v[q].y - gq.y) * d);
             }
         } else {
 #pragma unroll
             for (int q = 0; q < E; ++q) {
-                const T k2a = base2A + kl[q], k2b = base2B + kl[q];
-                const T da = s * rcp(T(1) + p.m.dtLke * k2a), db = s * rcp(T(1) + p.m.dtLke * k2b);
-                va[q] = cscale(va[q], da);
-                vb[q] = cscale(vb[q], db);
+                const T k2 = base2 + klast[j + q * TT];
+                v[q] = cscale(v[q], s * rcp(T(1) + p.m.dtLke * k2));
             }
         }
     }
@@ -211,12 +220,11 @@ col_kernel(const ColParams<T> p)
     if (ENERGY) {
         // sum over the full spectrum of |xi|^2 |u^|^2: columns with 0 < kx < M stand for their mirror too
         double acc = 0.0;
-        const double wa = (kxA == 0 || kxA == M) ? 1.0 : 2.0, wb = (kxB == 0 || kxB == M) ? 1.0 : 2.0;
-        const bool useA = valid && kxA <= M, useB = storeB && kxB <= M;
+        const double wgt = (kx == 0 || kx == M) ? 1.0 : 2.0;
+        if (store_ok && kx <= M) {
 #pragma unroll
-        for (int q = 0; q < E; ++q) {
-            if (useA) acc += wa * (double)(base2A + kl[q]) * ((double)va[q].x * va[q].x + (double)va[q].y * va[q].y);
-            if (useB) acc += wb * (double)(base2B + kl[q]) * ((double)vb[q].x * vb[q].x + (double)vb[q].y * vb[q].y);
+            for (int q = 0; q < E; ++q)
+                acc += wgt * (double)(base2 + klast[j + q * TT]) * ((double)v[q].x * v[q].x + (double)v[q].y * v[q].y);
         }
         double *red = reinterpret_cast<double *>(smem_raw);      // off the hot path: plain serial reduction
         __syncthreads();
@@ -231,36 +239,34 @@ col_kernel(const ColParams<T> p)
     }
 
     if (DO_INV) {
-        swap_all(va); swap_all(vb);
-        fft2_pipelined<N, E, 1, true>(va, vb, j, p.tw, bufA, bufB, bars);
-        swap_all(va); swap_all(vb);
-        if (!DO_UPD) {                                   // mid inverse: normalise here (the update folds 1/N in)
-            const T s = T(1) / T(N);
+        // inverse = swap re/im, forward, swap re/im (unnormalised; the update folds 1/N in)
 #pragma unroll
-            for (int q = 0; q < E; ++q) { va[q] = cscale(va[q], s); vb[q] = cscale(vb[q], s); }
-        }
+        for (int q = 0; q < E; ++q) v[q] = cswap(v[q]);
+        col_fft_forward<N, E>(v, j, p.tw, buf, sync);
+        const T s = DO_UPD ? T(1) : T(1) / T(N);
+#pragma unroll
+        for (int q = 0; q < E; ++q) v[q] = mk<T>(v[q].y * s, v[q].x * s);
     }
 
     if (PAIR_OUT) {
-        // E = (Ua + conj Ub)/2, W O = (Ua - conj Ub)/2, Z_a = E + i O, Z_b = conj(E - i O)
+        // E = (Ua + conj Ub)/2, W O = (Ua - conj Ub)/2, Z_a = E + i O, Z_b = conj(E - i O); the partner (other side
+        // of the pair) is the neighbouring lane
         const C wxc = cconj(wx);
+        C *dst = out + (side ? zcolB : zcolA);
 #pragma unroll
         for (int q = 0; q < E; ++q) {
-            const long i = j + q * TT;
-            const C e = mk<T>(T(0.5) * (va[q].x + vb[q].x), T(0.5) * (va[q].y - vb[q].y));
-            const C wo = mk<T>(T(0.5) * (va[q].x - vb[q].x), T(0.5) * (va[q].y + vb[q].y));
-            const C o = cmul(wxc, wo);
-            const C io = cmul_pi(o);
-            if (valid) out[i * p.out_rs + zcolA] = cadd(e, io);
-            if (storeB && zcolB != zcolA) out[i * p.out_rs + zcolB] = cconj(csub(e, io));
+            const C pv = shfl_xor1(v[q]);
+            const C ua = side ? pv : v[q], ubv = side ? v[q] : pv;
+            const C e = mk<T>(T(0.5) * (ua.x + ubv.x), T(0.5) * (ua.y - ubv.y));
+            const C wo = mk<T>(T(0.5) * (ua.x - ubv.x), T(0.5) * (ua.y + ubv.y));
+            const C io = cmul_pi(cmul(wxc, wo));
+            const C z = side ? cconj(csub(e, io)) : cadd(e, io);
+            if (store_ok) dst[(long)(j + q * TT) * p.out_rs] = z;
         }
     } else {
 #pragma unroll
-        for (int q = 0; q < E; ++q) {
-            const long i = j + q * TT;
-            if (valid) out[i * p.out_rs + pcolA] = va[q];
-            if (storeB) out[i * p.out_rs + pcolB] = vb[q];
-        }
+        for (int q = 0; q < E; ++q)
+            if (store_ok) out[(long)(j + q * TT) * p.out_rs + pcol] = v[q];
     }
 }
 
@@ -268,21 +274,19 @@ template <typename T, int N, int E, int TP, int MODE>
 static cudaError_t launch_col_inst(int nslots, int nbatch, const ColParams<T> &p, cudaStream_t s)
 {
     typedef typename V2<T>::type C;
-    constexpr int TT = N / E;
+    typedef ColShape<N, E, TP> Sh;
     constexpr bool PAIRS = (MODE == COL_2D_LAST || MODE == COL_3D_MIDFWD || MODE == COL_3D_MIDINV || MODE == COL_2D_ENERGY);
     constexpr bool DO_UPD = (MODE == COL_2D_LAST || MODE == COL_3D_LAST);
-    const int nblk = PAIRS ? (p.M / 2 + TP) / TP : p.ncols / (2 * TP);
-    const int gx = (DO_UPD && p.has_c) ? nblk : (nblk + 1) / 2;       // a c CTA covers one block of units, the others two
-    size_t smem = (size_t)2 * N * 2 * TP * sizeof(C);
-    ColParams<T> q = p;
-    q.bar_off = (int)smem;                   // 2 x 4 mbarriers behind the exchange buffers
-    smem += 64;
+    const int nblk = PAIRS ? (p.M / 2 + TP) / TP : p.ncols / Sh::SLOTS;
+    const int gx = (DO_UPD && p.has_c) ? nblk : (nblk + 1) / 2;       // a c CTA covers one block of columns, the others two
+    size_t smem = (size_t)2 * N * Sh::SLOTS * sizeof(C);
+    if (smem < (size_t)Sh::THREADS * sizeof(double)) smem = (size_t)Sh::THREADS * sizeof(double);   // energy reduction
     auto kern = col_kernel<T, N, E, TP, MODE>;
     if (smem > 48 * 1024) {
         cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
         if (e != cudaSuccess) return e;
     }
-    return launch_pdl(kern, dim3((unsigned)gx, (unsigned)nbatch, (unsigned)nslots), dim3(2 * TP * TT), smem, s, p.pdl != 0, q);
+    return launch_pdl(kern, dim3((unsigned)gx, (unsigned)nbatch, (unsigned)nslots), dim3(Sh::THREADS), smem, s, p.pdl != 0, p);
 }
 
 template <typename T, int N, int E, int TP>
@@ -299,24 +303,24 @@ static cudaError_t launch_col_mode(int mode, int nslots, int nbatch, const ColPa
     return cudaErrorInvalidValue;
 }
 
-// nfft = length of the FFT axis. TP (units per group) keeps a group at whole warps for short axes and the two
-// exchange buffers of a CTA within 128 KB for long ones.
+// nfft = length of the FFT axis. TP (column pairs per group) keeps a group at whole warps for short axes and the
+// two exchange buffers of a CTA within 128 KB for long ones.
 template <typename T> cudaError_t launch_col(int mode, int nfft, int nslots, int nbatch, const ColParams<T> &p, cudaStream_t s)
 {
     switch (nfft) {
 #ifndef PF_ONLY_N
-    case 16:   return launch_col_mode<T, 16, 8, 16>(mode, nslots, nbatch, p, s);
+    case 16:   return launch_col_mode<T, 16, 8, 8>(mode, nslots, nbatch, p, s);
     case 32:   return launch_col_mode<T, 32, 8, 8>(mode, nslots, nbatch, p, s);
-    case 64:   return launch_col_mode<T, 64, 8, 8>(mode, nslots, nbatch, p, s);
+    case 64:   return launch_col_mode<T, 64, 8, 4>(mode, nslots, nbatch, p, s);
     case 128:  return launch_col_mode<T, 128, 8, 4>(mode, nslots, nbatch, p, s);
     case 256:  return launch_col_mode<T, 256, 8, 4>(mode, nslots, nbatch, p, s);
-    case 512:  return launch_col_mode<T, 512, 8, 4>(mode, nslots, nbatch, p, s);
+    case 512:  return launch_col_mode<T, 512, 8, 2>(mode, nslots, nbatch, p, s);
 #endif
 #if !defined(PF_ONLY_N) || PF_ONLY_N == 1024
     case 1024: return launch_col_mode<T, 1024, 8, 2>(mode, nslots, nbatch, p, s);
 #endif
 #ifndef PF_ONLY_N
-    case 2048: return launch_col_mode<T, 2048, 16, 1>(mode, nslots, nbatch, p, s);
+    case 2048: return launch_col_mode<T, 2048, 8, 1>(mode, nslots, nbatch, p, s);
 #endif
     }
     return cudaErrorInvalidValue;

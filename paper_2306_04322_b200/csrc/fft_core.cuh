@@ -109,30 +109,49 @@ template <int R> struct Dft {
 __host__ __device__ constexpr int stage_radix(int N, int E, int NS) { return (N / NS < E) ? N / NS : E; }
 __host__ __device__ constexpr int num_stages(int N, int E) { int s = 0; for (int ns = 1; ns < N; ns *= stage_radix(N, E, ns)) ++s; return s; }
 
-// twiddle + butterflies of one stage on the E registers of thread j (see the header comment).
-// tw[i] = exp(-2 pi i * i / N), i in [0, N).
+// First twiddle W_{NS*R}^{k} of each of the S = E/R butterflies thread j owns in the stage that starts at NS
+// (k = butterfly index mod NS). Separated from the arithmetic so that a kernel can issue these table loads
+// ahead of the barrier that precedes the stage. tw[i] = exp(-2 pi i * i / N), i in [0, N).
+template <int N, int E, int NS> struct StageShape {
+    static constexpr int R = stage_radix(N, E, NS);
+    static constexpr int S = E / R;                   // butterflies per thread
+    static constexpr int TT = N / E;
+};
 template <int N, int E, int NS, typename C>
-PF_HD void stage_compute(C (&v)[E], int j, const C *__restrict__ tw)
+PF_HD void stage_twiddles(C (&w1)[StageShape<N, E, NS>::S], int j, const C *__restrict__ tw)
+{
+    typedef StageShape<N, E, NS> Sh;
+    if (NS > 1) {
+#pragma unroll
+        for (int m = 0; m < Sh::S; ++m) {
+            const int k = (j + m * Sh::TT) & (NS - 1);
+#if defined(__CUDA_ARCH__)
+            w1[m] = __ldg(tw + k * (N / (NS * Sh::R)));
+#else
+            w1[m] = tw[k * (N / (NS * Sh::R))];
+#endif
+        }
+    }
+}
+
+// twiddle + butterflies of one stage on the E registers of a thread (see the header comment); w1 from stage_twiddles.
+// Powers within a butterfly are formed by a balanced product tree.
+template <int N, int E, int NS, typename C>
+PF_HD void stage_compute_w(C (&v)[E], const C (&w1)[StageShape<N, E, NS>::S])
 {
 #ifdef PF_DBG_SKIP_COMPUTE
     return;
 #endif
-    constexpr int R = stage_radix(N, E, NS);
-    constexpr int S = E / R;                          // butterflies per thread
-    constexpr int TT = N / E;
+    constexpr int R = StageShape<N, E, NS>::R;
+    constexpr int S = StageShape<N, E, NS>::S;
 #pragma unroll
     for (int m = 0; m < S; ++m) {
         C a[R];
 #pragma unroll
         for (int r = 0; r < R; ++r) a[r] = v[m + r * S];
         if (NS > 1) {
-            const int k = (j + m * TT) & (NS - 1);
             C w[R];
-#if defined(__CUDA_ARCH__)
-            w[1] = __ldg(tw + k * (N / (NS * R)));
-#else
-            w[1] = tw[k * (N / (NS * R))];
-#endif
+            w[1] = w1[m];
 #pragma unroll
             for (int r = 2; r < R; ++r) w[r] = (r & 1) ? cmul(w[r / 2], w[r - r / 2]) : csqr(w[r / 2]);
 #pragma unroll
@@ -142,6 +161,15 @@ PF_HD void stage_compute(C (&v)[E], int j, const C *__restrict__ tw)
 #pragma unroll
         for (int r = 0; r < R; ++r) v[m + r * S] = a[r];
     }
+}
+
+// twiddle + butterflies of one stage on the E registers of thread j (table load at the point of use)
+template <int N, int E, int NS, typename C>
+PF_HD void stage_compute(C (&v)[E], int j, const C *__restrict__ tw)
+{
+    C w1[StageShape<N, E, NS>::S];
+    stage_twiddles<N, E, NS>(w1, j, tw);
+    stage_compute_w<N, E, NS>(v, w1);
 }
 
 // scatter the outputs of a non-final stage into the exchange buffer; buf(i) -> reference to element i

@@ -64,7 +64,6 @@ template <typename T> struct ColParams {
     const T *ky2;            // per ky (2D last: the FFT axis; 3D last: the middle axis)
     const T *kz2;            // per kz (3D last: the FFT axis)
     double  *acc;            // energy modes: accumulator (one double per field)
-    int      bar_off;        // byte offset of the mbarriers in dynamic shared memory (set by the launcher)
     Model<T> m;
 };
 
