@@ -46,36 +46,6 @@ struct GroupSync {
     __device__ __forceinline__ void operator()() const { asm volatile("bar.sync %0, %1;" ::"r"(id), "r"(n) : "memory"); }
 };
 
-// Forward transform of the column a thread shares with the TT-1 other threads of its slot. w1 = twiddles of the
-// stage that starts at NS; those of the next stage are requested between the two barriers of the exchange, when
-// the data registers are dead and the table latency hides behind the barrier.
-template <int N, int E, int NS, typename C, typename Buf>
-__device__ __forceinline__ void col_fft(C (&v)[E], int j, const C *__restrict__ tw, Buf &buf, const GroupSync &sync,
-                                        const C (&w1)[StageShape<N, E, NS>::S])
-{
-    stage_compute_w<N, E, NS>(v, w1);
-    constexpr int R = stage_radix(N, E, NS);
-    if constexpr (NS * R < N) {
-        C w2[StageShape<N, E, NS * R>::S];
-        sync();                                   // every thread has taken its elements of the previous exchange
-#ifndef PF_DBG_SKIP_EXCHANGE
-        buf.template store<N, E, NS>(v, j);
-#endif
-        stage_twiddles<N, E, NS * R>(w2, j, tw);
-        sync();
-#ifndef PF_DBG_SKIP_EXCHANGE
-        buf.template load<N, E>(v, j);
-#endif
-        col_fft<N, E, NS * R>(v, j, tw, buf, sync, w2);
-    }
-}
-template <int N, int E, typename C, typename Buf>
-__device__ __forceinline__ void col_fft_forward(C (&v)[E], int j, const C *__restrict__ tw, Buf &buf, const GroupSync &sync)
-{
-    C w0[StageShape<N, E, 1>::S];                 // first stage has no twiddles
-    col_fft<N, E, 1>(v, j, tw, buf, sync, w0);
-}
-
 template <int N, int E, int TP> struct ColShape {
     static constexpr int TT = N / E;
     static constexpr int SLOTS = 2 * TP;
@@ -184,7 +154,7 @@ col_kernel(const ColParams<T> p)
         for (int q = 0; q < E; ++q) v[q] = in[(long)(j + q * TT) * p.in_rs + pcol];
     }
 
-    if (DO_FWD) col_fft_forward<N, E>(v, j, p.tw, buf, sync);
+    if (DO_FWD) fft_forward<N, E>(v, j, p.tw, buf, sync);
 
     const T *klast = LAST3D ? p.kz2 : p.ky2;
 #ifndef PF_DBG_SKIP_UPDATE
@@ -242,7 +212,7 @@ col_kernel(const ColParams<T> p)
         // inverse = swap re/im, forward, swap re/im (unnormalised; the update folds 1/N in)
 #pragma unroll
         for (int q = 0; q < E; ++q) v[q] = cswap(v[q]);
-        col_fft_forward<N, E>(v, j, p.tw, buf, sync);
+        fft_forward<N, E>(v, j, p.tw, buf, sync);
         const T s = DO_UPD ? T(1) : T(1) / T(N);
 #pragma unroll
         for (int q = 0; q < E; ++q) v[q] = mk<T>(v[q].y * s, v[q].x * s);

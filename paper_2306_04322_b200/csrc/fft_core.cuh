@@ -203,38 +203,41 @@ PF_HD void exchange_load(C (&v)[E], int j, const Buf &buf)
 }
 
 #if defined(__CUDACC__)
-// Full forward transform of one column held by the TT threads that share `buf`; Sync()() must be a
-// barrier over (at least) those threads. Inverse = swap re/im, forward, swap re/im (unnormalised).
+// Full forward transform of one column held by the TT threads that share `buf`; sync() must be a barrier over (at
+// least) those threads. Inverse = swap re/im, forward, swap re/im (unnormalised). Buf provides
+// store<N, E, NS>(v, j) (Stockham scatter of a non-final stage) and load<N, E>(v, j) (elements j + q*TT).
+// w1 = twiddles of the stage that starts at NS; those of the next stage are requested between the two barriers
+// of the exchange, when the data registers are dead and the table latency hides behind the barrier.
 template <int N, int E, int NS, typename C, typename Buf, typename Sync>
-__device__ __forceinline__ void fft_stages(C (&v)[E], int j, const C *__restrict__ tw, Buf &buf, Sync &sync)
+__device__ __forceinline__ void fft_stages_w(C (&v)[E], int j, const C *__restrict__ tw, Buf &buf, const Sync &sync,
+                                             const C (&w1)[StageShape<N, E, NS>::S])
 {
-    stage_compute<N, E, NS>(v, j, tw);
+    stage_compute_w<N, E, NS>(v, w1);
     constexpr int R = stage_radix(N, E, NS);
     if constexpr (NS * R < N) {
+        C w2[StageShape<N, E, NS * R>::S];
+        sync();                                   // every thread has taken its elements of the previous exchange
+#ifndef PF_DBG_SKIP_EXCHANGE
+        buf.template store<N, E, NS>(v, j);
+#endif
+#ifndef PF_NO_TW_HOIST
+        stage_twiddles<N, E, NS * R>(w2, j, tw);
+#endif
         sync();
-        exchange_store<N, E, NS>(v, j, buf);
-        sync();
-        exchange_load<N, E>(v, j, buf);
-        fft_stages<N, E, NS * R>(v, j, tw, buf, sync);
+#ifdef PF_NO_TW_HOIST
+        stage_twiddles<N, E, NS * R>(w2, j, tw);
+#endif
+#ifndef PF_DBG_SKIP_EXCHANGE
+        buf.template load<N, E>(v, j);
+#endif
+        fft_stages_w<N, E, NS * R>(v, j, tw, buf, sync, w2);
     }
 }
-// Two independent columns A and B at once (one barrier pair per exchange for both; ILP of two).
-template <int N, int E, int NS, typename C, typename Buf, typename Sync>
-__device__ __forceinline__ void fft2_stages(C (&va)[E], C (&vb)[E], int j, const C *__restrict__ tw,
-                                            Buf &bufa, Buf &bufb, Sync &sync)
+template <int N, int E, typename C, typename Buf, typename Sync>
+__device__ __forceinline__ void fft_forward(C (&v)[E], int j, const C *__restrict__ tw, Buf &buf, const Sync &sync)
 {
-    stage_compute<N, E, NS>(va, j, tw);
-    stage_compute<N, E, NS>(vb, j, tw);
-    constexpr int R = stage_radix(N, E, NS);
-    if constexpr (NS * R < N) {
-        sync();
-        exchange_store<N, E, NS>(va, j, bufa);
-        exchange_store<N, E, NS>(vb, j, bufb);
-        sync();
-        exchange_load<N, E>(va, j, bufa);
-        exchange_load<N, E>(vb, j, bufb);
-        fft2_stages<N, E, NS * R>(va, vb, j, tw, bufa, bufb, sync);
-    }
+    C w0[StageShape<N, E, 1>::S];                 // the first stage has no twiddles; never read
+    fft_stages_w<N, E, 1>(v, j, tw, buf, sync, w0);
 }
 template <int E, typename C> __device__ __forceinline__ void swap_all(C (&v)[E])
 {
@@ -244,82 +247,3 @@ template <int E, typename C> __device__ __forceinline__ void swap_all(C (&v)[E])
 #endif
 
 }  // namespace pf
-
-#if defined(__CUDACC__)
-namespace pf {
-
-// ---------------------------------------------------------------------------------------------------
-// Split (arrive / wait) CTA barriers on shared-memory mbarriers, one arrival per warp. They let the two
-// columns A and B that a thread owns run half a stage out of phase: while a warp waits for "all of A has
-// been stored", other warps are still in the butterflies of B, so the fp64 pipe and the shared-memory
-// pipe are busy at the same time instead of alternating between CTA-wide barriers.
-// Four barriers: ready/free for the A slots and for the B slots of the exchange buffer.
-// ---------------------------------------------------------------------------------------------------
-struct PipeBars {
-    unsigned base;      // shared-memory address of 4 x 8 bytes
-    unsigned par;       // expected parity per barrier (bit b = barrier b)
-    enum { READY_A = 0, FREE_A = 1, READY_B = 2, FREE_B = 3 };
-
-    // the caller follows this with a barrier over the threads that will use the object
-    __device__ __forceinline__ void init(void *smem4x8, int nwarps, bool init_thread)
-    {
-        base = (unsigned)__cvta_generic_to_shared(smem4x8);
-        par = (1u << FREE_A) | (1u << FREE_B);        // "free" passes the first time (nothing to wait for)
-        if (init_thread) {
-#pragma unroll
-            for (int b = 0; b < 4; ++b)
-                asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(base + 8 * b), "r"(nwarps) : "memory");
-        }
-    }
-    __device__ __forceinline__ void arrive(int b)
-    {
-        __syncwarp();
-        if ((threadIdx.x & 31) == 0)
-            asm volatile("{\n\t.reg .b64 st;\n\tmbarrier.arrive.shared::cta.b64 st, [%0];\n\t}" ::"r"(base + 8 * b) : "memory");
-    }
-    __device__ __forceinline__ void wait(int b)
-    {
-        const unsigned addr = base + 8 * b, p = (par >> b) & 1u;
-        asm volatile(
-            "{\n\t.reg .pred P1;\n\t"
-            "WAIT_LOOP:\n\t"
-            "mbarrier.try_wait.parity.shared::cta.b64 P1, [%0], %1;\n\t"
-            "@P1 bra DONE;\n\t"
-            "bra WAIT_LOOP;\n\t"
-            "DONE:\n\t}" ::"r"(addr), "r"(p) : "memory");
-        par ^= 1u << b;
-    }
-};
-
-// Forward transform of the two columns a thread owns, software pipelined over the stage boundaries.
-template <int N, int E, int NS, bool FIRST, typename C, typename Buf>
-__device__ __forceinline__ void fft2_pipelined(C (&va)[E], C (&vb)[E], int j, const C *__restrict__ tw,
-                                               Buf &bufa, Buf &bufb, PipeBars &bars)
-{
-    constexpr int R = stage_radix(N, E, NS);
-    constexpr bool LAST = !(NS * R < N);
-    stage_compute<N, E, NS>(va, j, tw);
-    if constexpr (!LAST) {
-        bars.wait(PipeBars::FREE_A);
-        exchange_store<N, E, NS>(va, j, bufa);
-        bars.arrive(PipeBars::READY_A);
-    }
-    if constexpr (!FIRST) {
-        bars.wait(PipeBars::READY_B);
-        exchange_load<N, E>(vb, j, bufb);
-        bars.arrive(PipeBars::FREE_B);
-    }
-    stage_compute<N, E, NS>(vb, j, tw);
-    if constexpr (!LAST) {
-        bars.wait(PipeBars::FREE_B);
-        exchange_store<N, E, NS>(vb, j, bufb);
-        bars.arrive(PipeBars::READY_B);
-        bars.wait(PipeBars::READY_A);
-        exchange_load<N, E>(va, j, bufa);
-        bars.arrive(PipeBars::FREE_A);
-        fft2_pipelined<N, E, NS * R, false>(va, vb, j, tw, bufa, bufb, bars);
-    }
-}
-
-}  // namespace pf
-#endif

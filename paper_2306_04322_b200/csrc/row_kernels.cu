@@ -25,6 +25,8 @@ template <typename C, int LOGPAD> struct RowBuf {
     C *base;
     __device__ __forceinline__ void st(int i, C v) { base[i + (i >> LOGPAD)] = v; }
     __device__ __forceinline__ C ld(int i) const { return base[i + (i >> LOGPAD)]; }
+    template <int N, int E, int NS> __device__ __forceinline__ void store(const C (&v)[E], int j) { exchange_store<N, E, NS>(v, j, *this); }
+    template <int N, int E> __device__ __forceinline__ void load(C (&v)[E], int j) const { exchange_load<N, E>(v, j, *this); }
 };
 struct CtaSync { __device__ __forceinline__ void operator()() const { __syncthreads(); } };
 
@@ -55,7 +57,7 @@ __global__ void __maxnreg__((M >= 256) ? 80 : 64) row_kernel(const RowParams<T> 
     const long row = (long)blockIdx.x * RB + r;
     const bool valid = row < p.nrows;
     RowBuf<C, 3> buf{smem + (long)rf * MP};
-    CtaSync sync;
+    const CtaSync sync;
 
     grid_dependency_wait();
     grid_dependents_launch();
@@ -69,7 +71,7 @@ __global__ void __maxnreg__((M >= 256) ? 80 : 64) row_kernel(const RowParams<T> 
         const C *src = p.zst + f * p.zfs + row * M;
 #pragma unroll
         for (int q = 0; q < E; ++q) v[q] = valid ? cswap(src[j + q * TT]) : mk<T>(0, 0);   // swap: inverse via forward
-        fft_stages<M, E, 1>(v, j, p.tw, buf, sync);
+        fft_forward<M, E>(v, j, p.tw, buf, sync);
         const T s = T(1) / T(M);
 #pragma unroll
         for (int q = 0; q < E; ++q) v[q] = mk<T>(v[q].y * s, v[q].x * s);                    // swap back, normalise
@@ -115,7 +117,7 @@ __global__ void __maxnreg__((M >= 256) ? 80 : 64) row_kernel(const RowParams<T> 
         }
     }
 
-    fft_stages<M, E, 1>(v, j, p.tw, buf, sync);
+    fft_forward<M, E>(v, j, p.tw, buf, sync);
 
     C *dst = (MODE == ROW_STEP && f == 0) ? (p.zg + row * M) : (p.zst + f * p.zfs + row * M);
     if (valid) {
