@@ -1,15 +1,15 @@
 // col_kernels.cu -- strided-direction kernels of the Fourier-spectral step.
 //
-// A CTA is two independent thread GROUPS; a group owns SLOTS = 2*TP adjacent columns and all N elements of each
-// along the FFT axis. Thread (slot, j) of a group holds elements j + q*TT (q < E, TT = N/E) of ONE column in
-// registers (fft_core.cuh), before and after every transform, so the pointwise work is register local. The slot
-// is the fastest thread index: consecutive lanes own consecutive columns, every global access of a warp is made
-// of contiguous 16*SLOTS-byte (fp64) pieces, and the strided "transpose" happens in registers plus one
-// shared-memory exchange per FFT stage boundary (col_buf.cuh). A group synchronises on its own named barrier, so
-// the groups of a CTA and the CTAs of an SM drift apart and overlap each other's memory, shared-memory and fp64
-// phases; one column per thread keeps the kernel at 64 registers, i.e. 32 resident warps per SM.
+// A CTA owns SLOTS = 2*TP adjacent columns and all N elements of each along the FFT axis. Thread (slot, j) holds
+// elements j + q*TT (q < E, TT = N/E) of ONE column in registers (fft_core.cuh), before and after every transform,
+// so the pointwise work is register local. The slot is the fastest thread index: consecutive lanes own consecutive
+// columns, every global access of a warp is made of contiguous 16*SLOTS-byte (fp64) pieces, and the strided
+// "transpose" happens in registers plus one shared-memory exchange per FFT stage boundary (col_buf.cuh). One column
+// per thread keeps the kernel at 64 registers and N*SLOTS*16 bytes of shared memory per CTA (64 KB at N = 1024), so
+// two to four CTAs share an SM, start and finish at different times, and one CTA's loads and stores overlap the
+// transforms of the others.
 //
-// In the pair modes the columns of a group are TP mirror pairs (u, M-u) of the z-form (row_kernels.cu): with
+// In the pair modes the columns of a CTA are TP mirror pairs (u, M-u) of the z-form (row_kernels.cu): with
 //   E = (Z_u + conj Z_{M-u})/2,  O = -(i/2)(Z_u - conj Z_{M-u}),  W = exp(-2 pi i u / nx)
 // the true half-spectrum columns are  U_u = E + W O  (side 0) and  U_{M-u} = conj(E - W O)  (side 1), pointwise
 // along the column; u = 0 yields the DC and Nyquist columns from Z_0 alone and u = M/2 is its own mirror. Both
@@ -19,10 +19,9 @@
 //   eta^ <- w^ / ( 1 + dt L kappa_eta |xi|^2 ),  w = eta - dt L h        Eqs. 13, 15
 // with |xi|^2 = kx2 + ky2 (+ kz2) from 1-D tables (Eq. 16/19 or the FS-FD variants).
 //
-// Field slots (blockIdx.z): in the update modes slot 0 is c, whose CTA uses its two groups for the two arrays the
-// update needs on the SAME columns: group 0 transforms g = df/dc, scales it by dt M |xi|^2 and hands it over
-// through shared memory; group 1 transforms c^, combines, inverts and stores. Every other CTA uses its two groups
-// for two consecutive blocks of columns of one array.
+// Field slots (blockIdx.z): in the update modes slot 0 is c, which needs two forward transforms on the same columns:
+// its CTAs first transform g = df/dc, scale it by dt M |xi|^2 and park it in global memory (each thread reads back
+// what it wrote itself; the 8 MB stay in L2), then transform c^, combine, invert and store.
 #include "pf_kernels.cuh"
 #include "col_buf.cuh"
 
@@ -40,18 +39,13 @@ __device__ __forceinline__ float2 shfl_xor1(float2 v)
     return make_float2(__shfl_xor_sync(0xffffffffu, v.x, 1), __shfl_xor_sync(0xffffffffu, v.y, 1));
 }
 
-// named barrier over the threads of one group (id 0 is __syncthreads)
-struct GroupSync {
-    int id, n;
-    __device__ __forceinline__ void operator()() const { asm volatile("bar.sync %0, %1;" ::"r"(id), "r"(n) : "memory"); }
-};
+struct CtaSync { __device__ __forceinline__ void operator()() const { __syncthreads(); } };
 
 template <int N, int E, int TP> struct ColShape {
     static constexpr int TT = N / E;
     static constexpr int SLOTS = 2 * TP;
-    static constexpr int GT = SLOTS * TT;                               // threads per group (whole warps)
-    static constexpr int THREADS = 2 * GT;
-    static constexpr int MINB = (THREADS >= 1024) ? 1 : 1024 / THREADS;  // 64 registers per thread
+    static constexpr int THREADS = SLOTS * TT;                           // whole warps
+    static constexpr int MINB = (THREADS >= 1024) ? 1 : ((1024 / THREADS > 32) ? 32 : 1024 / THREADS);   // 64 registers
     static constexpr int LR = (E >= 16) ? 4 : 3;                         // log2 of the first-stage radix
 };
 
@@ -64,7 +58,7 @@ col_kernel(const ColParams<T> p)
 #endif
     typedef typename V2<T>::type C;
     typedef ColShape<N, E, TP> Sh;
-    constexpr int TT = Sh::TT, SLOTS = Sh::SLOTS, GT = Sh::GT;
+    constexpr int TT = Sh::TT, SLOTS = Sh::SLOTS, GT = Sh::THREADS;
     constexpr bool PAIRS = (MODE == COL_2D_LAST || MODE == COL_3D_MIDFWD || MODE == COL_3D_MIDINV || MODE == COL_2D_ENERGY);
     constexpr bool PAIR_IN = (MODE == COL_2D_LAST || MODE == COL_3D_MIDFWD || MODE == COL_2D_ENERGY);
     constexpr bool PAIR_OUT = (MODE == COL_2D_LAST || MODE == COL_3D_MIDINV);
@@ -73,26 +67,24 @@ col_kernel(const ColParams<T> p)
     constexpr bool DO_UPD = (MODE == COL_2D_LAST || MODE == COL_3D_LAST);
     constexpr bool DO_INV = (MODE == COL_2D_LAST || MODE == COL_3D_LAST || MODE == COL_3D_MIDINV);
     constexpr bool LAST3D = (MODE == COL_3D_LAST || MODE == COL_3D_ENERGY);
-    static_assert(GT % 32 == 0, "a group must be whole warps");
+    static_assert(GT % 32 == 0, "a CTA must be whole warps");
 
     extern __shared__ __align__(16) unsigned char smem_raw[];
-    const int g = threadIdx.x / GT;                    // group
-    const int tg = threadIdx.x - g * GT;
-    const int sl = tg % SLOTS;                         // column slot: side = sl & 1, unit t = sl >> 1
+    const int tid = threadIdx.x;
+    const int sl = tid % SLOTS;                        // column slot: side = sl & 1, pair t = sl >> 1
     const int side = sl & 1;
-    const int j = tg / SLOTS;
+    const int j = tid / SLOTS;
     const int M = p.M;
     const int slot = blockIdx.z;                       // field slot
     const long bz = blockIdx.y;
+    const int ub = blockIdx.x;                         // block of SLOTS columns
     const bool c_cta = DO_UPD && p.has_c && slot == 0;
 
-    ColBuf<C, SLOTS, Sh::LR> buf{reinterpret_cast<C *>(smem_raw) + (long)g * N * SLOTS, sl};
-    const GroupSync sync{1 + g, GT};
+    ColBuf<C, SLOTS, Sh::LR> buf{reinterpret_cast<C *>(smem_raw), sl};
+    const CtaSync sync;
 
-    // ---- which block of columns, which column ----
-    const int nblk = PAIRS ? (M / 2 + TP) / TP : p.ncols / SLOTS;
-    const int ub = c_cta ? (int)blockIdx.x : 2 * (int)blockIdx.x + g;
-    bool valid = ub < nblk;
+    // ---- which column ----
+    bool valid = true;
     bool store_ok;                        // this thread writes its column
     int zcolA = 0, zcolB = 0;             // z-form columns of the pair (pitch M)
     int pcol = 0;                         // column index in plain arrays (half-spectrum planes)
@@ -101,7 +93,7 @@ col_kernel(const ColParams<T> p)
     C wx = mk<T>(1, 0);                   // exp(-2 pi i u / nx)
     if (PAIRS) {
         int u = ub * TP + (sl >> 1);
-        valid = valid && (u <= M / 2);
+        valid = (u <= M / 2);
         if (!valid) u = 0;
         zcolA = u; zcolB = (M - u) & (M - 1);
         kx = side ? M - u : u;
@@ -110,19 +102,17 @@ col_kernel(const ColParams<T> p)
         wx = p.twx[u];
         base2 = p.kx2[kx];
     } else {
-        pcol = (valid ? ub : 0) * SLOTS + sl;
-        store_ok = valid;
+        pcol = ub * SLOTS + sl;
+        store_ok = true;
         kx = pcol % p.P2;
         base2 = p.kx2[kx] + p.ky2[pcol / p.P2];
     }
-    // a CTA whose two groups both have no columns leaves (eta slots are launched with the c slot's grid)
-    if (!ENERGY && __syncthreads_or(valid) == 0) return;
 
-    // ---- arrays of this CTA / group ----
+    // ---- arrays of this CTA ----
     const C *in;
     C *out;
     if (c_cta) {
-        in = (g == 0) ? p.in1 : p.in0;
+        in = p.in1;                        // first pass: g = df/dc
         out = p.out;
     } else if (slot == 0 && p.alt_in) {
         in = p.alt_in; out = p.alt_out;
@@ -134,47 +124,52 @@ col_kernel(const ColParams<T> p)
     out += bz * p.out_bs;
 
     C v[E];
+    auto load_columns = [&](const C *src) {
+        if (PAIR_IN) {
+#pragma unroll
+            for (int q = 0; q < E; ++q) {
+                const long i = j + q * TT;
+                const C za = src[i * p.in_rs + zcolA], zb = src[i * p.in_rs + zcolB];
+                // E = (za + conj zb)/2, O = -(i/2)(za - conj zb)
+                const C e = mk<T>(T(0.5) * (za.x + zb.x), T(0.5) * (za.y - zb.y));
+                const C o = mk<T>(T(0.5) * (za.y + zb.y), T(-0.5) * (za.x - zb.x));
+                const C wo = cmul(wx, o);
+                v[q] = side ? cconj(csub(e, wo)) : cadd(e, wo);
+            }
+        } else {
+#pragma unroll
+            for (int q = 0; q < E; ++q) v[q] = src[(long)(j + q * TT) * p.in_rs + pcol];
+        }
+    };
 
     grid_dependency_wait();                // everything above touches constant tables only
     grid_dependents_launch();
 
-    if (PAIR_IN) {
+    const T *klast = LAST3D ? p.kz2 : p.ky2;
+    C *park = nullptr;
+    if (c_cta) {
+        // Cahn-Hilliard needs two transforms on the same columns: dt M |xi|^2 g^ is formed first and parked in
+        // global memory (thread-linear: written and read back by the same thread, L2 resident), then c^ follows.
+        park = p.park + ((bz * gridDim.x + ub) * (long)E) * GT + tid;
+        load_columns(in);
+        fft_forward<N, E>(v, j, p.tw, buf, sync);
 #pragma unroll
-        for (int q = 0; q < E; ++q) {
-            const long i = j + q * TT;
-            const C za = in[i * p.in_rs + zcolA], zb = in[i * p.in_rs + zcolB];
-            // E = (za + conj zb)/2, O = -(i/2)(za - conj zb)
-            const C e = mk<T>(T(0.5) * (za.x + zb.x), T(0.5) * (za.y - zb.y));
-            const C o = mk<T>(T(0.5) * (za.y + zb.y), T(-0.5) * (za.x - zb.x));
-            const C wo = cmul(wx, o);
-            v[q] = side ? cconj(csub(e, wo)) : cadd(e, wo);
-        }
-    } else {
-#pragma unroll
-        for (int q = 0; q < E; ++q) v[q] = in[(long)(j + q * TT) * p.in_rs + pcol];
+        for (int q = 0; q < E; ++q) park[(long)q * GT] = cscale(v[q], p.m.dtM * (base2 + klast[j + q * TT]));
+        in = p.in0 + bz * p.in_bs;
     }
 
+    load_columns(in);
     if (DO_FWD) fft_forward<N, E>(v, j, p.tw, buf, sync);
 
-    const T *klast = LAST3D ? p.kz2 : p.ky2;
 #ifndef PF_DBG_SKIP_UPDATE
     if (DO_UPD) {
         const T s = T(1) / T(N);
         if (c_cta) {
-            // group 0: dt M |xi|^2 g^ -> shared memory (thread-linear in its own buffer) -> group 1
-            C *hand = reinterpret_cast<C *>(smem_raw);
-            if (g == 0) {
-                sync();                                              // group 0 has left its exchange buffer
-#pragma unroll
-                for (int q = 0; q < E; ++q) hand[q * GT + tg] = cscale(v[q], p.m.dtM * (base2 + klast[j + q * TT]));
-            }
-            __syncthreads();
-            if (g == 0) return;
 #pragma unroll
             for (int q = 0; q < E; ++q) {
                 const T k2 = base2 + klast[j + q * TT];
                 const T d = s * rcp(T(1) + p.m.dtMkc * k2 * k2);
-                const C gq = hand[q * GT + tg];
+                const C gq = park[(long)q * GT];
                 v[q] = mk<T>((v[q].x - gq.x) * d, (v[q].y - gq.y) * d);
             }
         } else {
@@ -198,11 +193,11 @@ col_kernel(const ColParams<T> p)
         }
         double *red = reinterpret_cast<double *>(smem_raw);      // off the hot path: plain serial reduction
         __syncthreads();
-        red[threadIdx.x] = acc;
+        red[tid] = acc;
         __syncthreads();
-        if (threadIdx.x == 0) {
+        if (tid == 0) {
             double tot = 0.0;
-            for (int w = 0; w < 2 * GT; ++w) tot += red[w];
+            for (int w = 0; w < GT; ++w) tot += red[w];
             atomicAdd(p.acc + slot, tot);
         }
         return;
@@ -246,10 +241,8 @@ static cudaError_t launch_col_inst(int nslots, int nbatch, const ColParams<T> &p
     typedef typename V2<T>::type C;
     typedef ColShape<N, E, TP> Sh;
     constexpr bool PAIRS = (MODE == COL_2D_LAST || MODE == COL_3D_MIDFWD || MODE == COL_3D_MIDINV || MODE == COL_2D_ENERGY);
-    constexpr bool DO_UPD = (MODE == COL_2D_LAST || MODE == COL_3D_LAST);
-    const int nblk = PAIRS ? (p.M / 2 + TP) / TP : p.ncols / Sh::SLOTS;
-    const int gx = (DO_UPD && p.has_c) ? nblk : (nblk + 1) / 2;       // a c CTA covers one block of columns, the others two
-    size_t smem = (size_t)2 * N * Sh::SLOTS * sizeof(C);
+    const int gx = PAIRS ? (p.M / 2 + TP) / TP : p.ncols / Sh::SLOTS;    // blocks of SLOTS columns
+    size_t smem = (size_t)N * Sh::SLOTS * sizeof(C);
     if (smem < (size_t)Sh::THREADS * sizeof(double)) smem = (size_t)Sh::THREADS * sizeof(double);   // energy reduction
     auto kern = col_kernel<T, N, E, TP, MODE>;
     if (smem > 48 * 1024) {

@@ -7,6 +7,7 @@
 //   zg       [nz][ny][M]    complex z-form of g = df/dc
 //   s2       [F][nz][ny][P2] complex, 3D only: (kx,ky)-spectral, z-real planes; s2[0] carries c between steps
 //   g2       [nz][ny][P2]   complex, 3D only
+//   park     [nz][ny][P2+16] complex scratch of the column kernels (dt M |xi|^2 g^ of the Cahn-Hilliard update)
 //   mu       [N]            FD chemical potential
 //   tables   twiddles exp(-2 pi i k/n) for M, ny, nz, nx; |xi_d|^2 per axis (Eq. 16-21)
 #include <cmath>
@@ -39,7 +40,7 @@ struct pf_ctx {
     bool graph_ok = true;
     void *real[2] = {nullptr, nullptr};
     int cur = 0;
-    void *zst = nullptr, *zg = nullptr, *s2 = nullptr, *g2 = nullptr, *mu = nullptr;
+    void *zst = nullptr, *zg = nullptr, *s2 = nullptr, *g2 = nullptr, *mu = nullptr, *park = nullptr;
     void *tw_m = nullptr, *tw_y = nullptr, *tw_z = nullptr, *tw_nx = nullptr;
     void *kx2 = nullptr, *ky2 = nullptr, *kz2 = nullptr;
     double *acc = nullptr;
@@ -163,6 +164,7 @@ template <typename T> ColParams<T> col_params(pf_ctx *c)
     q.twx = (const C *)c->tw_nx;
     q.kx2 = (const T *)c->kx2; q.ky2 = (const T *)c->ky2; q.kz2 = (const T *)c->kz2;
     q.acc = c->acc;
+    q.park = (C *)c->park;
     q.m = make_model<T>(c->p);
     return q;
 }
@@ -412,7 +414,7 @@ void pf_destroy(pf_ctx *c)
     if (!c) return;
     drop_graph(c);
     for (auto &e : c->pev) if (e) cudaEventDestroy(e);
-    void *bufs[] = {c->real[0], c->real[1], c->zst, c->zg, c->s2, c->g2, c->mu, c->tw_m, c->tw_y, c->tw_z,
+    void *bufs[] = {c->real[0], c->real[1], c->zst, c->zg, c->s2, c->g2, c->mu, c->park, c->tw_m, c->tw_y, c->tw_z,
                     c->tw_nx, c->kx2, c->ky2, c->kz2, c->acc};
     for (void *b : bufs) if (b) cudaFree(b);
     if (c->own_stream) cudaStreamDestroy(c->stream);
@@ -461,7 +463,8 @@ int pf_create(const pf_params *p, pf_ctx **out)
     int rc;
     if ((rc = alloc(&c->real[0], fb * c->F)) || (rc = alloc(&c->real[1], fb * c->F)) ||
         (rc = alloc(&c->zst, fb * c->F)) || (rc = alloc(&c->zg, fb)) || (rc = alloc(&c->mu, fb)) ||
-        (rc = alloc((void **)&c->acc, sizeof(double) * 32)))
+        (rc = alloc((void **)&c->acc, sizeof(double) * 32)) ||
+        (rc = alloc(&c->park, (size_t)(c->P2 + 16) * c->p.n[1] * c->p.n[2] * 2 * c->w)))
         return fail(rc);
     if (p->ndim == 3) {
         const size_t pb = (size_t)c->p.n[2] * c->p.n[1] * c->P2 * 2 * c->w;

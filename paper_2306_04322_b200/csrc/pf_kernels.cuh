@@ -48,6 +48,7 @@ template <typename T> struct ColParams {
     const C *in0;            // input of slot s: in0 + s*in_fs  (eta fields: w = eta - dt L h; slot 0: the c state)
     const C *in1;            // update modes with has_c: g = df/dc (same layout as slot 0 of in0)
     C       *out;            // output of slot s: out + s*out_fs
+    C       *park;           // update modes with has_c: scratch for dt M |xi|^2 g^, one complex per spectral mode (+ padding)
     const C *alt_in;         // if non-null, slot 0 reads alt_in and writes alt_out instead (3D y-forward of g)
     C       *alt_out;
     int      has_c;          // update modes: slot 0 is the Cahn-Hilliard field (needs in1)
