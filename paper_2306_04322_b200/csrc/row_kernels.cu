@@ -17,6 +17,7 @@
 // Thread layout: block = RB rows x F fields x TT = M/E threads; thread (r, f, j) owns elements
 // j + q*TT of the transform of field f of row r (fft_core.cuh). One barrier-separated shared-memory
 // exchange per FFT stage boundary plus one for the nonlinear coupling.
+#include <type_traits>
 #include "pf_kernels.cuh"
 
 namespace pf {
@@ -29,6 +30,11 @@ template <typename C, int LOGPAD> struct RowBuf {
     template <int N, int E> __device__ __forceinline__ void load(C (&v)[E], int j) const { exchange_load<N, E>(v, j, *this); }
 };
 struct CtaSync { __device__ __forceinline__ void operator()() const { __syncthreads(); } };
+// a transform carried by exactly one warp exchanges through its own buffer: warp-level synchronisation is enough,
+// and the warps of an SM drift apart (their fp64 and shared-memory phases overlap instead of alternating)
+struct WarpSync { __device__ __forceinline__ void operator()() const { __syncwarp(); } };
+template <int TT> struct FftSync { typedef typename std::conditional<(TT <= 32), WarpSync, CtaSync>::type type; };
+
 
 template <int M, int E> __host__ __device__ constexpr int row_pitch() { return M + (M >> 3) + 1; }
 
@@ -36,7 +42,7 @@ template <int M, int E> __host__ __device__ constexpr int row_pitch() { return M
 // than the last few registers (measured on B200: 94 -> 80 registers: 1024^2 row kernel 28.1 -> 26.4 us; 64 at
 // nx = 256: 394 -> 317 us at 256^3).
 template <typename T, int M, int E, int MODE>
-__global__ void __maxnreg__((M >= 256) ? 80 : 64) row_kernel(const RowParams<T> p)
+__global__ void __maxnreg__((E >= 16) ? 128 : (M >= 256) ? 80 : 64) row_kernel(const RowParams<T> p)
 {
 #ifdef PF_DBG_EMPTY
     return;
@@ -58,6 +64,7 @@ __global__ void __maxnreg__((M >= 256) ? 80 : 64) row_kernel(const RowParams<T> 
     const bool valid = row < p.nrows;
     RowBuf<C, 3> buf{smem + (long)rf * MP};
     const CtaSync sync;
+    const typename FftSync<TT>::type fsync;
 
     grid_dependency_wait();
     grid_dependents_launch();
@@ -71,7 +78,7 @@ __global__ void __maxnreg__((M >= 256) ? 80 : 64) row_kernel(const RowParams<T> 
         const C *src = p.zst + f * p.zfs + row * M;
 #pragma unroll
         for (int q = 0; q < E; ++q) v[q] = valid ? cswap(src[j + q * TT]) : mk<T>(0, 0);   // swap: inverse via forward
-        fft_forward<M, E>(v, j, p.tw, buf, sync);
+        fft_forward<M, E>(v, j, p.tw, buf, fsync);
         const T s = T(1) / T(M);
 #pragma unroll
         for (int q = 0; q < E; ++q) v[q] = mk<T>(v[q].y * s, v[q].x * s);                    // swap back, normalise
@@ -117,7 +124,9 @@ __global__ void __maxnreg__((M >= 256) ? 80 : 64) row_kernel(const RowParams<T> 
         }
     }
 
-    fft_forward<M, E>(v, j, p.tw, buf, sync);
+    // with warp-level exchange barriers the buffers the other fields' threads have just read need a CTA barrier
+    if (MODE == ROW_STEP && TT <= 32) sync();
+    fft_forward<M, E>(v, j, p.tw, buf, fsync);
 
     C *dst = (MODE == ROW_STEP && f == 0) ? (p.zg + row * M) : (p.zst + f * p.zfs + row * M);
     if (valid) {
