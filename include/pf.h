@@ -101,7 +101,11 @@ long long pf_launch_count(const pf_ctx *ctx);
 /* Device time in milliseconds spent by kernel `which` of the most recent pf_step_fs call, measured
  * with CUDA events on the context's stream when profiling was switched on with pf_set_profiling
  * (which = 0 .. pf_num_fs_kernels()-1, in launch order within one step; averaged over the steps of
- * that call). Returns a negative value when unavailable. Profiling disables CUDA-graph replay. */
+ * that call). Returns a negative value when unavailable. Profiling disables CUDA-graph replay.
+ * pf_set_profiling(ctx, R): R = 0 switches it off; R = 1 brackets every kernel of a step with events; R > 1 launches
+ * every kernel R times back to back between its two events and reports elapsed / R, which removes the event and
+ * launch overhead from the per-kernel figure -- the fields are then NOT a valid trajectory (each kernel was applied
+ * R times): call pf_set_fields before stepping again. */
 int    pf_set_profiling(pf_ctx *ctx, int on);
 int    pf_num_fs_kernels(const pf_ctx *ctx);
 double pf_fs_kernel_ms(pf_ctx *ctx, int which);

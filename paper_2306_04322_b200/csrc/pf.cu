@@ -52,7 +52,7 @@ struct pf_ctx {
     cudaGraphExec_t fs_graph = nullptr;
     int fs_graph_nodes = 0;
     // profiling
-    bool profiling = false;
+    int profiling = 0;                   // 0 off; R >= 1: events around every kernel, each launched R times back to back
     int nk = 0;
     const char *kname[kMaxFsKernels] = {};
     double kms[kMaxFsKernels] = {};
@@ -198,6 +198,7 @@ template <typename T> cudaError_t mid_forward(pf_ctx *c, const void *zsrc, long 
 // stream serialization: each kernel's prologue overlaps its predecessor's tail (griddepcontrol in the kernels).
 template <typename T> int fs_one_step(pf_ctx *c, cudaEvent_t *events)
 {
+    const int rep = events ? (c->profiling > 1 ? c->profiling : 1) : 1;
     typedef typename V2<T>::type C;
     const int ny = c->p.n[1], nz = c->p.n[2];
     const long zfs = c->N / 2;
@@ -205,7 +206,8 @@ template <typename T> int fs_one_step(pf_ctx *c, cudaEvent_t *events)
     KernelTimer kt(c, events);
     RowParams<T> r = row_params<T>(c);
     r.pdl = pdl;
-    PF_CK(c, launch_row<T>(ROW_STEP, c->p.n[0], r, c->stream)); ++c->launches; kt.mark("row_c2r_nonlinear_r2c");
+    for (int i = 0; i < rep; ++i) { PF_CK(c, launch_row<T>(ROW_STEP, c->p.n[0], r, c->stream)); ++c->launches; }
+    kt.mark("row_c2r_nonlinear_r2c");
     C *zst = (C *)c->zst;
     if (c->p.ndim == 2) {
         ColParams<T> q = col_params<T>(c);
@@ -213,23 +215,27 @@ template <typename T> int fs_one_step(pf_ctx *c, cudaEvent_t *events)
         q.in_rs = q.out_rs = c->M;
         q.in0 = zst; q.in1 = (const C *)c->zg; q.out = zst; q.in_fs = q.out_fs = zfs;
         q.has_c = 1; q.pdl = pdl;
-        PF_CK(c, launch_col<T>(COL_2D_LAST, ny, c->F, 1, q, c->stream)); ++c->launches; kt.mark("col_y_fft_update_ifft");
+        for (int i = 0; i < rep; ++i) { PF_CK(c, launch_col<T>(COL_2D_LAST, ny, c->F, 1, q, c->stream)); ++c->launches; }
+        kt.mark("col_y_fft_update_ifft");
     } else {
         const long s2fs = (long)nz * ny * c->P2;
         C *s2 = (C *)c->s2;
-        PF_CK(c, mid_forward<T>(c, zst, zfs, s2, s2fs, c->F, true, pdl)); kt.mark("col_y_fwd");
+        for (int i = 0; i < rep; ++i) PF_CK(c, mid_forward<T>(c, zst, zfs, s2, s2fs, c->F, true, pdl));
+        kt.mark("col_y_fwd");
         ColParams<T> q = col_params<T>(c);
         q.tw = (const C *)c->tw_z;
         q.in_rs = q.out_rs = (long)ny * c->P2; q.ncols = ny * c->P2;
         q.in0 = s2; q.in1 = (const C *)c->g2; q.out = s2; q.in_fs = q.out_fs = s2fs;
         q.has_c = 1; q.pdl = pdl;
-        PF_CK(c, launch_col<T>(COL_3D_LAST, nz, c->F, 1, q, c->stream)); ++c->launches; kt.mark("col_z_fft_update_ifft");
+        for (int i = 0; i < rep; ++i) { PF_CK(c, launch_col<T>(COL_3D_LAST, nz, c->F, 1, q, c->stream)); ++c->launches; }
+        kt.mark("col_z_fft_update_ifft");
         ColParams<T> v = col_params<T>(c);
         v.tw = (const C *)c->tw_y;
         v.in0 = s2; v.in_fs = s2fs; v.in_rs = c->P2; v.in_bs = (long)ny * c->P2;
         v.out = zst; v.out_fs = zfs; v.out_rs = c->M; v.out_bs = (long)ny * c->M;
         v.pdl = pdl;
-        PF_CK(c, launch_col<T>(COL_3D_MIDINV, ny, c->F, nz, v, c->stream)); ++c->launches; kt.mark("col_y_inv");
+        for (int i = 0; i < rep; ++i) { PF_CK(c, launch_col<T>(COL_3D_MIDINV, ny, c->F, nz, v, c->stream)); ++c->launches; }
+        kt.mark("col_y_inv");
     }
     c->nk = kt.k;
     return PF_OK;
@@ -284,7 +290,7 @@ template <typename T> int step_fs(pf_ctx *c, int nsteps)
                     sum[k] += ms;
                 }
         }
-        for (int k = 0; k < c->nk; ++k) c->kms[k] = sum[k] / nsteps;
+        for (int k = 0; k < c->nk; ++k) c->kms[k] = sum[k] / nsteps / (c->profiling > 1 ? c->profiling : 1);
     } else {
         // replay one captured step; small grids are launch-latency bound without it
         if (!c->fs_graph && c->graph_ok) {
@@ -542,7 +548,7 @@ long long pf_launch_count(const pf_ctx *c) { return c ? c->launches : 0; }
 int pf_set_profiling(pf_ctx *c, int on)
 {
     if (!c) return PF_EINVAL;
-    c->profiling = on != 0;
+    c->profiling = on > 0 ? on : 0;
     for (double &v : c->kms) v = -1.0;
     return PF_OK;
 }

@@ -20,6 +20,11 @@
 #include <type_traits>
 #include "pf_kernels.cuh"
 
+#ifndef PF_ROW_REGS_BIG
+#define PF_ROW_REGS_BIG 80
+#endif
+#define PF_ROW_REGS(M, E) (((E) >= 16) ? 128 : ((M) >= 256) ? PF_ROW_REGS_BIG : 64)
+
 namespace pf {
 
 template <typename C, int LOGPAD> struct RowBuf {
@@ -42,7 +47,7 @@ template <int M, int E> __host__ __device__ constexpr int row_pitch() { return M
 // than the last few registers (measured on B200: 94 -> 80 registers: 1024^2 row kernel 28.1 -> 26.4 us; 64 at
 // nx = 256: 394 -> 317 us at 256^3).
 template <typename T, int M, int E, int MODE>
-__global__ void __maxnreg__((E >= 16) ? 128 : (M >= 256) ? 80 : 64) row_kernel(const RowParams<T> p)
+__global__ void __maxnreg__(PF_ROW_REGS(M, E)) row_kernel(const RowParams<T> p)
 {
 #ifdef PF_DBG_EMPTY
     return;

@@ -166,8 +166,10 @@ class Context:
     def launch_count(self) -> int:
         return int(lib().pf_launch_count(self._h))
 
-    def set_profiling(self, on: bool):
-        self._ck(lib().pf_set_profiling(self._h, int(bool(on))), "pf_set_profiling")
+    def set_profiling(self, repeat):
+        """0/False: off; 1/True: events around every kernel; R > 1: every kernel launched R times between its events
+        (timing only: the fields are not a valid trajectory afterwards, see pf.h)."""
+        self._ck(lib().pf_set_profiling(self._h, int(repeat)), "pf_set_profiling")
 
     def fs_kernel_times(self):
         """[(name, ms)] of the most recent profiled pf_step_fs call."""
