@@ -25,6 +25,17 @@
 #include "pf_kernels.cuh"
 #include "col_buf.cuh"
 
+// column pairs per CTA at the longer axes (tuned on B200)
+#ifndef PF_TP_256
+#define PF_TP_256 4
+#endif
+#ifndef PF_TP_512
+#define PF_TP_512 2
+#endif
+#ifndef PF_TP_2048
+#define PF_TP_2048 2
+#endif
+
 namespace pf {
 
 __device__ __forceinline__ double rcp(double x) { return __drcp_rn(x); }
@@ -276,14 +287,14 @@ template <typename T> cudaError_t launch_col(int mode, int nfft, int nslots, int
     case 32:   return launch_col_mode<T, 32, 8, 8>(mode, nslots, nbatch, p, s);
     case 64:   return launch_col_mode<T, 64, 8, 4>(mode, nslots, nbatch, p, s);
     case 128:  return launch_col_mode<T, 128, 8, 4>(mode, nslots, nbatch, p, s);
-    case 256:  return launch_col_mode<T, 256, 8, 4>(mode, nslots, nbatch, p, s);
-    case 512:  return launch_col_mode<T, 512, 8, 2>(mode, nslots, nbatch, p, s);
+    case 256:  return launch_col_mode<T, 256, 8, PF_TP_256>(mode, nslots, nbatch, p, s);
+    case 512:  return launch_col_mode<T, 512, 8, PF_TP_512>(mode, nslots, nbatch, p, s);
 #endif
 #if !defined(PF_ONLY_N) || PF_ONLY_N == 1024
     case 1024: return launch_col_mode<T, 1024, 8, 2>(mode, nslots, nbatch, p, s);
 #endif
 #ifndef PF_ONLY_N
-    case 2048: return launch_col_mode<T, 2048, 8, 1>(mode, nslots, nbatch, p, s);
+    case 2048: return launch_col_mode<T, 2048, 8, PF_TP_2048>(mode, nslots, nbatch, p, s);
 #endif
     }
     return cudaErrorInvalidValue;

@@ -3,8 +3,13 @@
 //
 // Paper form: kernel (i) mu = df/dc - kappa_c lap c, kernel (ii) c' = c + dt M lap mu, kernel (iii)
 // eta_i' = eta_i - dt L (df/deta_i - kappa_eta lap eta_i); 2nd-order centred 5-point (2D) / 7-point (3D)
-// Laplacian, periodic boundaries, every right-hand side at time t. Here (ii) and (iii) are one launch
-// and the ghost layers are replaced by wrap-around index arithmetic (no ghost storage).
+// Laplacian, periodic boundaries, every right-hand side at time t. The ghost layers are replaced by wrap-around
+// index arithmetic (no ghost storage).
+//   2D: ONE launch per step. A CTA stages a TX x TY tile in shared memory -- c with a halo of two points, every
+//       eta_i with a halo of one -- forms mu on the tile plus a ring of one point (kernel (i)), and from that
+//       the new c and eta_i of the tile (kernels (ii), (iii)): each field is read once and written once per step,
+//       2(p+1) R bytes instead of the (3p+5) R of the separate kernels (the halo re-reads stay in L1/L2).
+//   3D: kernels (i) and (ii)+(iii) as two launches on global memory (neighbours served by L1/L2).
 #include "pf_kernels.cuh"
 
 namespace pf {
@@ -65,6 +70,62 @@ template <typename T> __global__ void fd_update_kernel(const FdParams<T> p)
     }
 }
 
+// 2D fused step, see the header. Dynamic shared memory: c tile (TY+4) x (TX+4), mu tile (TY+2) x (TX+2),
+// n_eta tiles (TY+2) x (TX+2). nx, ny are powers of two >= TX, TY.
+template <typename T, int TX, int TY>
+__global__ void __launch_bounds__(256) fd_fused2d_kernel(const FdParams<T> p)
+{
+    constexpr int CW = TX + 4, CH = TY + 4, EW = TX + 2, EH = TY + 2;
+    extern __shared__ __align__(16) unsigned char fd_smem[];
+    T *sc = reinterpret_cast<T *>(fd_smem);
+    T *smu = sc + CW * CH;
+    T *se = smu + EW * EH;
+    const int x0 = blockIdx.x * TX, y0 = blockIdx.y * TY;
+    const int mx = p.nx - 1, my = p.ny - 1;
+    const int ne = p.m.n_eta;
+
+    for (int i = threadIdx.x; i < CW * CH; i += blockDim.x) {
+        const int lx = i % CW, ly = i / CW;
+        sc[i] = p.c[(long)((y0 + ly - 2) & my) * p.nx + ((x0 + lx - 2) & mx)];
+    }
+    for (int i = threadIdx.x; i < EW * EH; i += blockDim.x) {
+        const int lx = i % EW, ly = i / EW;
+        const long g = (long)((y0 + ly - 1) & my) * p.nx + ((x0 + lx - 1) & mx);
+        for (int k = 0; k < ne; ++k) se[k * (EW * EH) + i] = p.eta[(long)k * p.N + g];
+    }
+    __syncthreads();
+
+    // kernel (i) on the tile and its ring: mu = df_chem/dc - kappa_c lap c
+    for (int i = threadIdx.x; i < EW * EH; i += blockDim.x) {
+        const int lx = i % EW, ly = i / EW;
+        const T *cc = sc + (ly + 1) * CW + (lx + 1);
+        const T v = cc[0];
+        const T l = p.rdx2[0] * (cc[1] + cc[-1] - T(2) * v) + p.rdx2[1] * (cc[CW] + cc[-CW] - T(2) * v);
+        T h = 0;
+        for (int k = 0; k < ne; ++k) h += h_term(se[k * (EW * EH) + i]);
+        smu[i] = dfdc(p.m, v, h) - p.m.kappa_c * l;
+    }
+    __syncthreads();
+
+    // kernels (ii) + (iii) on the tile
+    for (int i = threadIdx.x; i < TX * TY; i += blockDim.x) {
+        const int lx = i % TX, ly = i / TX;
+        const long g = (long)(y0 + ly) * p.nx + (x0 + lx);
+        const int e0 = (ly + 1) * EW + (lx + 1);
+        const T c = sc[(ly + 2) * CW + (lx + 2)];
+        const T *mu = smu + e0;
+        const T lm = p.rdx2[0] * (mu[1] + mu[-1] - T(2) * mu[0]) + p.rdx2[1] * (mu[EW] + mu[-EW] - T(2) * mu[0]);
+        p.c_new[g] = c + p.m.dtM * lm;
+        T s2 = 0;
+        for (int k = 0; k < ne; ++k) { const T e = se[k * (EW * EH) + e0]; s2 += e * e; }
+        for (int k = 0; k < ne; ++k) {
+            const T *e = se + k * (EW * EH) + e0;
+            const T le = p.rdx2[0] * (e[1] + e[-1] - T(2) * e[0]) + p.rdx2[1] * (e[EW] + e[-EW] - T(2) * e[0]);
+            p.eta_new[(long)k * p.N + g] = e[0] - p.m.dtL * (dfdeta(p.m, c, e[0], s2) - p.m.kappa_eta * le);
+        }
+    }
+}
+
 // Eq. 1 pieces in real space: acc[0] += sum f_chem, acc[1] += sum |grad c|^2, acc[2+i] += sum |grad eta_i|^2
 // (forward differences when gradient_kind == 1). Accumulated in fp64; scaled by the caller.
 template <typename T> __global__ void energy_kernel(const EnergyParams<T> p)
@@ -121,6 +182,24 @@ template <typename T> cudaError_t launch_fd_update(const FdParams<T> &p, cudaStr
     fd_update_kernel<T><<<(unsigned)((p.N + 255) / 256), 256, 0, s>>>(p);
     return cudaGetLastError();
 }
+template <typename T, int TX, int TY> static cudaError_t launch_fd_fused2d_inst(const FdParams<T> &p, cudaStream_t s)
+{
+    const size_t smem = sizeof(T) * ((size_t)(TX + 4) * (TY + 4) + (size_t)(1 + p.m.n_eta) * (TX + 2) * (TY + 2));
+    auto kern = fd_fused2d_kernel<T, TX, TY>;
+    if (smem > 48 * 1024) {
+        cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        if (e != cudaSuccess) return e;
+    }
+    kern<<<dim3((unsigned)(p.nx / TX), (unsigned)(p.ny / TY)), 256, smem, s>>>(p);
+    return cudaGetLastError();
+}
+// one fused launch per 2D step (nz == 1)
+template <typename T> cudaError_t launch_fd_fused2d(const FdParams<T> &p, cudaStream_t s)
+{
+    if (p.nx >= 64) return launch_fd_fused2d_inst<T, 64, 16>(p, s);
+    if (p.nx >= 32) return launch_fd_fused2d_inst<T, 32, 16>(p, s);
+    return launch_fd_fused2d_inst<T, 16, 16>(p, s);
+}
 template <typename T> cudaError_t launch_energy(const EnergyParams<T> &p, cudaStream_t s)
 {
     long blocks = (p.N + 255) / 256;
@@ -133,6 +212,8 @@ template cudaError_t launch_fd_mu<double>(const FdParams<double> &, cudaStream_t
 template cudaError_t launch_fd_mu<float>(const FdParams<float> &, cudaStream_t);
 template cudaError_t launch_fd_update<double>(const FdParams<double> &, cudaStream_t);
 template cudaError_t launch_fd_update<float>(const FdParams<float> &, cudaStream_t);
+template cudaError_t launch_fd_fused2d<double>(const FdParams<double> &, cudaStream_t);
+template cudaError_t launch_fd_fused2d<float>(const FdParams<float> &, cudaStream_t);
 template cudaError_t launch_energy<double>(const EnergyParams<double> &, cudaStream_t);
 template cudaError_t launch_energy<float>(const EnergyParams<float> &, cudaStream_t);
 

@@ -332,9 +332,14 @@ template <typename T> int step_fd(pf_ctx *c, int nsteps)
     for (int s = 0; s < nsteps; ++s) {
         T *cu = (T *)c->real[c->cur], *nw = (T *)c->real[c->cur ^ 1];
         f.c = cu; f.eta = cu + c->N; f.c_new = nw; f.eta_new = nw + c->N;
-        PF_CK(c, launch_fd_mu<T>(f, c->stream));
-        PF_CK(c, launch_fd_update<T>(f, c->stream));
-        c->launches += 2;
+        if (c->p.ndim == 2) {
+            PF_CK(c, launch_fd_fused2d<T>(f, c->stream));
+            c->launches += 1;
+        } else {
+            PF_CK(c, launch_fd_mu<T>(f, c->stream));
+            PF_CK(c, launch_fd_update<T>(f, c->stream));
+            c->launches += 2;
+        }
         c->cur ^= 1;
     }
     c->state = ST_REAL;

@@ -94,6 +94,7 @@ template <typename T> cudaError_t launch_row(int mode, int nx, const RowParams<T
 template <typename T> cudaError_t launch_col(int mode, int nfft, int nslots, int nbatch, const ColParams<T> &p, cudaStream_t s);
 template <typename T> cudaError_t launch_fd_mu(const FdParams<T> &p, cudaStream_t s);
 template <typename T> cudaError_t launch_fd_update(const FdParams<T> &p, cudaStream_t s);
+template <typename T> cudaError_t launch_fd_fused2d(const FdParams<T> &p, cudaStream_t s);
 template <typename T> cudaError_t launch_energy(const EnergyParams<T> &p, cudaStream_t s);
 
 #if defined(__CUDACC__)

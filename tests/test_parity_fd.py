@@ -25,6 +25,17 @@ def test_fd_c1_noise_dx1(oracle):
     assert rel_linf([gc, geta], [rc, reta]) < 1e-12
 
 
+@pytest.mark.parametrize("n,n_eta,steps", [((16, 16), 1, 50), ((32, 16), 8, 30), ((1024, 1024), 2, 20), ((2048, 64), 4, 20)])
+def test_fd_fused_2d_tiles(oracle, n, n_eta, steps):
+    # the fused shared-memory-halo kernel: smallest tiles (TX = 16, 32), most fields, and the crossover size
+    # (configs[4] grid, 64 x 64 tiles of 64 x 16 points, halos wrapping in both directions)
+    c, eta, dx = make_init("B", n, n_eta)
+    kt2 = sum(4.0 / d ** 2 for d in dx)
+    dt = min(0.75 * 2.0 / (5.0 * kt2 * (4.0 + 3.0 * kt2)), 2e-3)
+    (gc, geta), (rc, reta) = run_both(oracle, n=n, n_eta=n_eta, init="B", steps=steps, dt=dt, method="fd")
+    assert rel_linf([gc, geta], [rc, reta]) < 1e-12
+
+
 def test_fd_fp32(oracle):
     (gc, geta), (rc, reta) = run_both(oracle, n=(64, 64), n_eta=2, init="B", steps=200, dt=1e-3, method="fd", precision="f32")
     assert rel_linf([gc, geta], [rc, reta]) < 1e-4

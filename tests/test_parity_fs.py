@@ -64,6 +64,32 @@ def test_large_1024_sq(oracle):
     _check(oracle, TOL64, n=(1024, 1024), n_eta=2, init="B", steps=5, dt=5e-3)
 
 
+def test_c4_256_cubed_two_steps_and_invariants(oracle):
+    # BASELINE.json configs[3] at full size in the launch configuration bench.py times: element-wise parity after 2
+    # steps (the oracle needs seconds per step), then properties that hold at any length: mean c conserved
+    # (Eq. 14 leaves the k = 0 mode untouched) and the free energy does not increase
+    from paper_2306_04322_b200 import pf, synth
+    n, p = (256, 256, 256), 2
+    _check(oracle, TOL64, n=n, n_eta=p, init="B", steps=2, dt=5e-3)
+    c, eta, dx = synth.init_b(n, p)
+    with pf.Context(n, n_eta=p, dx=dx, dt=5e-3) as ctx:
+        ctx.set_fields(c, eta)
+        e_prev = ctx.free_energy(0)[0]
+        for _ in range(3):
+            ctx.step_fs(10)
+            e = ctx.free_energy(0)[0]
+            assert e <= e_prev * (1 + 1e-12)
+            e_prev = e
+        gc, _ = ctx.get_fields()
+    assert abs(gc.mean() - c.mean()) < 1e-13
+
+
+def test_c3_2048_sq_p4(oracle):
+    # BASELINE.json configs[2]: 2048 x 2048, c + 4 eta, fp64 and fp32 side by side (3 steps; the oracle is slow here)
+    _check(oracle, TOL64, n=(2048, 2048), n_eta=4, init="B", steps=3, dt=5e-3)
+    _check(oracle, TOL32, n=(2048, 2048), n_eta=4, init="B", steps=3, dt=5e-3, precision="f32")
+
+
 def test_long_axes_2048(oracle):
     _check(oracle, TOL64, n=(2048, 32), n_eta=1, init="B", steps=10, dt=5e-3)
     _check(oracle, TOL64, n=(32, 2048), n_eta=1, init="B", steps=10, dt=5e-3)
