@@ -20,6 +20,9 @@
 #include <type_traits>
 #include "pf_kernels.cuh"
 
+#ifndef PF_ROW_E1024
+#define PF_ROW_E1024 8
+#endif
 #ifndef PF_ROW_REGS_BIG
 #define PF_ROW_REGS_BIG 80
 #endif
@@ -182,7 +185,7 @@ template <typename T> cudaError_t launch_row(int mode, int nx, const RowParams<T
     case 128:  return launch_row_mode<T, 128, 8>(mode, p, s);
     case 256:  return launch_row_mode<T, 256, 8>(mode, p, s);
     case 512:  return launch_row_mode<T, 512, 8>(mode, p, s);
-    case 1024: return launch_row_mode<T, 1024, 16>(mode, p, s);
+    case 1024: return launch_row_mode<T, 1024, PF_ROW_E1024>(mode, p, s);
     }
     return cudaErrorInvalidValue;
 }
