@@ -1,7 +1,7 @@
 #!/usr/bin/env python
 """bench.py -- throughput of the Fourier-spectral (FS) step of arXiv 2306.04322 on B200.
 
-    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload 1024sq|256cube|2048sq|2048sq_f32|512sq|64sq]
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload 1024sq|256cube|2048sq|2048sq_f32|512sq|256sq|64sq]
                     [--impl ours|reference]
 
 A "step" is one FS time step (all kernels of SURVEY 8(a): x-pass with the nonlinear evaluation, strided passes with
@@ -31,9 +31,10 @@ WORKLOADS = {
     "2048sq": ((2048, 2048), 4, "f64", "B", 5e-3, "2D 2048x2048, c + 4 eta, fp64 (configs[2])"),
     "2048sq_f32": ((2048, 2048), 4, "f32", "B", 5e-3, "2D 2048x2048, c + 4 eta, fp32 (configs[2])"),
     "512sq": ((512, 512), 4, "f64", "B", 5e-3, "2D 512x512, c + 4 eta, fp64 (configs[1] grid)"),
+    "256sq": ((256, 256), 4, "f64", "B", 5e-3, "2D 256x256, c + 4 eta, fp64 (paper Table 1 grid; its FS run of PAPER.md:286)"),
     "64sq": ((64, 64), 2, "f64", "A", 0.05, "2D 64x64, c + 2 eta, fp64 (configs[0])"),
 }
-DEFAULT_STEPS = {"1024sq": 20000, "256cube": 1500, "2048sq": 3000, "2048sq_f32": 5000, "512sq": 40000, "64sq": 100000}
+DEFAULT_STEPS = {"1024sq": 20000, "256cube": 1500, "2048sq": 3000, "2048sq_f32": 5000, "512sq": 40000, "256sq": 60000, "64sq": 100000}
 L2_BYTES = 126e6
 PROF_REPEAT = 8
 METRIC = "FS steps/s (Gpoint-updates/s and achieved HBM GB/s alongside)"

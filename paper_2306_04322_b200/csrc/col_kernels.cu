@@ -26,6 +26,15 @@
 #include "col_buf.cuh"
 
 // column pairs per CTA at the longer axes (tuned on B200)
+#ifndef PF_TP_32
+#define PF_TP_32 8
+#endif
+#ifndef PF_TP_64
+#define PF_TP_64 4
+#endif
+#ifndef PF_TP_128
+#define PF_TP_128 4
+#endif
 #ifndef PF_TP_256
 #define PF_TP_256 4
 #endif
@@ -284,9 +293,9 @@ template <typename T> cudaError_t launch_col(int mode, int nfft, int nslots, int
     switch (nfft) {
 #ifndef PF_ONLY_N
     case 16:   return launch_col_mode<T, 16, 8, 8>(mode, nslots, nbatch, p, s);
-    case 32:   return launch_col_mode<T, 32, 8, 8>(mode, nslots, nbatch, p, s);
-    case 64:   return launch_col_mode<T, 64, 8, 4>(mode, nslots, nbatch, p, s);
-    case 128:  return launch_col_mode<T, 128, 8, 4>(mode, nslots, nbatch, p, s);
+    case 32:   return launch_col_mode<T, 32, 8, PF_TP_32>(mode, nslots, nbatch, p, s);
+    case 64:   return launch_col_mode<T, 64, 8, PF_TP_64>(mode, nslots, nbatch, p, s);
+    case 128:  return launch_col_mode<T, 128, 8, PF_TP_128>(mode, nslots, nbatch, p, s);
     case 256:  return launch_col_mode<T, 256, 8, PF_TP_256>(mode, nslots, nbatch, p, s);
     case 512:  return launch_col_mode<T, 512, 8, PF_TP_512>(mode, nslots, nbatch, p, s);
 #endif

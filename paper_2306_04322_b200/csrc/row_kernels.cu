@@ -151,6 +151,7 @@ static cudaError_t launch_row_inst(const RowParams<T> &p, cudaStream_t s)
     const int per_row = TT * p.F;
     if (per_row > 1024) return cudaErrorInvalidConfiguration;
     int RB = 256 / per_row;
+    if (RB > p.nrows / 296) RB = p.nrows / 296;      // small grids: at least two CTAs per SM before rows are batched
     if (RB < 1) RB = 1;
     if (RB > p.nrows) RB = p.nrows;
     const int threads = RB * per_row;
