@@ -12,9 +12,21 @@
 //   3D: kernels (i) and (ii)+(iii) as two launches on global memory (neighbours served by L1/L2).
 #include "pf_kernels.cuh"
 
+#ifndef PF_FD_TY
+#define PF_FD_TY 16
+#endif
+
 namespace pf {
 
 struct Nbr { long xm, xp, ym, yp, zm, zp; };
+
+// global -> shared copy of one element without a register stop-over (LDGSTS): a thread queues all of its tile
+// elements at once and waits once, so a CTA has its whole tile in flight
+template <typename T> __device__ __forceinline__ void cp_async_elem(T *smem_dst, const T *gmem_src)
+{
+    asm volatile("cp.async.ca.shared.global [%0], [%1], %2;" ::"r"((unsigned)__cvta_generic_to_shared(smem_dst)), "l"(gmem_src), "n"(sizeof(T)) : "memory");
+}
+__device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_all;" ::: "memory"); }
 
 __device__ __forceinline__ Nbr neighbours(long i, int nx, int ny, int nz)
 {
@@ -72,7 +84,7 @@ template <typename T> __global__ void fd_update_kernel(const FdParams<T> p)
 
 // 2D fused step, see the header. Dynamic shared memory: c tile (TY+4) x (TX+4), mu tile (TY+2) x (TX+2),
 // n_eta tiles (TY+2) x (TX+2). nx, ny are powers of two >= TX, TY.
-template <typename T, int TX, int TY>
+template <typename T, int TX, int TY, int NE>
 __global__ void __launch_bounds__(256) fd_fused2d_kernel(const FdParams<T> p)
 {
     constexpr int CW = TX + 4, CH = TY + 4, EW = TX + 2, EH = TY + 2;
@@ -82,34 +94,50 @@ __global__ void __launch_bounds__(256) fd_fused2d_kernel(const FdParams<T> p)
     T *se = smu + EW * EH;
     const int x0 = blockIdx.x * TX, y0 = blockIdx.y * TY;
     const int mx = p.nx - 1, my = p.ny - 1;
-    const int ne = p.m.n_eta;
+    constexpr int ne = NE;                 // compile-time field count: the per-field loops unroll into fixed offsets
 
-    for (int i = threadIdx.x; i < CW * CH; i += blockDim.x) {
-        const int lx = i % CW, ly = i / CW;
-        sc[i] = p.c[(long)((y0 + ly - 2) & my) * p.nx + ((x0 + lx - 2) & mx)];
+    // thread (tx, ty) of TX x (256/TX): column tx (+ the halo columns for the first lanes), rows ty, ty + TYS, ..
+    constexpr int TYS = 256 / TX;
+    const int tx = threadIdx.x % TX, ty = threadIdx.x / TX;
+    grid_dependency_wait();
+    grid_dependents_launch();
+
+    for (int ly = ty; ly < CH; ly += TYS) {
+        const T *row = p.c + (long)((y0 + ly - 2) & my) * p.nx;
+        cp_async_elem(sc + ly * CW + tx, row + ((x0 + tx - 2) & mx));
+        if (tx < 4) cp_async_elem(sc + ly * CW + TX + tx, row + ((x0 + TX + tx - 2) & mx));
     }
-    for (int i = threadIdx.x; i < EW * EH; i += blockDim.x) {
-        const int lx = i % EW, ly = i / EW;
-        const long g = (long)((y0 + ly - 1) & my) * p.nx + ((x0 + lx - 1) & mx);
-        for (int k = 0; k < ne; ++k) se[k * (EW * EH) + i] = p.eta[(long)k * p.N + g];
+    for (int k = 0; k < ne; ++k) {
+        const T *ek = p.eta + (long)k * p.N;
+        T *sk = se + k * (EW * EH);
+        for (int ly = ty; ly < EH; ly += TYS) {
+            const T *row = ek + (long)((y0 + ly - 1) & my) * p.nx;
+            cp_async_elem(sk + ly * EW + tx, row + ((x0 + tx - 1) & mx));
+            if (tx < 2) cp_async_elem(sk + ly * EW + TX + tx, row + ((x0 + TX + tx - 1) & mx));
+        }
     }
+    cp_async_wait_all();
     __syncthreads();
 
     // kernel (i) on the tile and its ring: mu = df_chem/dc - kappa_c lap c
-    for (int i = threadIdx.x; i < EW * EH; i += blockDim.x) {
-        const int lx = i % EW, ly = i / EW;
+    auto mu_at = [&](int lx, int ly) {
+        const int i = ly * EW + lx;
         const T *cc = sc + (ly + 1) * CW + (lx + 1);
         const T v = cc[0];
         const T l = p.rdx2[0] * (cc[1] + cc[-1] - T(2) * v) + p.rdx2[1] * (cc[CW] + cc[-CW] - T(2) * v);
         T h = 0;
         for (int k = 0; k < ne; ++k) h += h_term(se[k * (EW * EH) + i]);
         smu[i] = dfdc(p.m, v, h) - p.m.kappa_c * l;
+    };
+    for (int ly = ty; ly < EH; ly += TYS) {
+        mu_at(tx, ly);
+        if (tx < 2) mu_at(TX + tx, ly);
     }
     __syncthreads();
 
     // kernels (ii) + (iii) on the tile
-    for (int i = threadIdx.x; i < TX * TY; i += blockDim.x) {
-        const int lx = i % TX, ly = i / TX;
+    for (int ly = ty; ly < TY; ly += TYS) {
+        const int lx = tx;
         const long g = (long)(y0 + ly) * p.nx + (x0 + lx);
         const int e0 = (ly + 1) * EW + (lx + 1);
         const T c = sc[(ly + 2) * CW + (lx + 2)];
@@ -182,22 +210,38 @@ template <typename T> cudaError_t launch_fd_update(const FdParams<T> &p, cudaStr
     fd_update_kernel<T><<<(unsigned)((p.N + 255) / 256), 256, 0, s>>>(p);
     return cudaGetLastError();
 }
-template <typename T, int TX, int TY> static cudaError_t launch_fd_fused2d_inst(const FdParams<T> &p, cudaStream_t s)
+template <typename T, int TX, int TY, int NE> static cudaError_t launch_fd_fused2d_ne(const FdParams<T> &p, cudaStream_t s)
 {
-    const size_t smem = sizeof(T) * ((size_t)(TX + 4) * (TY + 4) + (size_t)(1 + p.m.n_eta) * (TX + 2) * (TY + 2));
-    auto kern = fd_fused2d_kernel<T, TX, TY>;
+    const size_t smem = sizeof(T) * ((size_t)(TX + 4) * (TY + 4) + (size_t)(1 + NE) * (TX + 2) * (TY + 2));
+    auto kern = fd_fused2d_kernel<T, TX, TY, NE>;
     if (smem > 48 * 1024) {
         cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
         if (e != cudaSuccess) return e;
     }
-    kern<<<dim3((unsigned)(p.nx / TX), (unsigned)(p.ny / TY)), 256, smem, s>>>(p);
-    return cudaGetLastError();
+    // programmatic dependent launch: consecutive steps cannot overlap, but the launch latency of step t+1 hides
+    // behind the tail of step t
+    return launch_pdl(kern, dim3((unsigned)(p.nx / TX), (unsigned)(p.ny / TY)), dim3(256), smem, s, true, p);
+}
+template <typename T, int TX, int TY> static cudaError_t launch_fd_fused2d_inst(const FdParams<T> &p, cudaStream_t s)
+{
+    switch (p.m.n_eta) {
+    case 0: return launch_fd_fused2d_ne<T, TX, TY, 0>(p, s);
+    case 1: return launch_fd_fused2d_ne<T, TX, TY, 1>(p, s);
+    case 2: return launch_fd_fused2d_ne<T, TX, TY, 2>(p, s);
+    case 3: return launch_fd_fused2d_ne<T, TX, TY, 3>(p, s);
+    case 4: return launch_fd_fused2d_ne<T, TX, TY, 4>(p, s);
+    case 5: return launch_fd_fused2d_ne<T, TX, TY, 5>(p, s);
+    case 6: return launch_fd_fused2d_ne<T, TX, TY, 6>(p, s);
+    case 7: return launch_fd_fused2d_ne<T, TX, TY, 7>(p, s);
+    case 8: return launch_fd_fused2d_ne<T, TX, TY, 8>(p, s);
+    }
+    return cudaErrorInvalidValue;
 }
 // one fused launch per 2D step (nz == 1)
 template <typename T> cudaError_t launch_fd_fused2d(const FdParams<T> &p, cudaStream_t s)
 {
-    if (p.nx >= 64) return launch_fd_fused2d_inst<T, 64, 16>(p, s);
-    if (p.nx >= 32) return launch_fd_fused2d_inst<T, 32, 16>(p, s);
+    if (p.nx >= 64) return launch_fd_fused2d_inst<T, 64, PF_FD_TY>(p, s);
+    if (p.nx >= 32) return launch_fd_fused2d_inst<T, 32, PF_FD_TY>(p, s);
     return launch_fd_fused2d_inst<T, 16, 16>(p, s);
 }
 template <typename T> cudaError_t launch_energy(const EnergyParams<T> &p, cudaStream_t s)
