@@ -349,6 +349,25 @@ def run_ours(args):
             "l2_resident_single_simulation": {"value": resident, "unit": "steps/s", "gpoint_updates_per_s": resident * N / 1e9},
             "roofline": roofline, "step_roofline": step_roofline, "e2e": e2e, "gpu_launches": int(launches), "clocks": clocks}
 
+    # comparison path: explicit FD steps of one simulation of the same grid, device-timed
+    fd = pf.Context(n, n_eta=p, dx=dx, dt=1e-6, precision=prec, stream=stream.cuda_stream)
+    fd.set_fields(c0, eta0)
+    kfd = max(20, min(2000, K // 4))
+    fd.step_fd(20)
+    f0, f1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    barrier()
+    f0.record(stream)
+    fd.step_fd(kfd)
+    f1.record(stream)
+    barrier()
+    fd_ms = f0.elapsed_time(f1) / kfd
+    fd.close()
+    fd_bytes = 2 * F * R if len(n) == 2 else (3 * p + 5) * R
+    line["fd_comparison_path"] = {"value": 1e3 / fd_ms, "unit": "steps/s", "us_per_step": 1e3 * fd_ms, "steps": kfd,
+                                  "algorithmic_bytes_per_step": fd_bytes, "achieved_gbs": fd_bytes / (fd_ms * 1e-3) / 1e9,
+                                  "note": "explicit forward-Euler 5/7-point step (pf_step_fd), single simulation (L2 resident below ~60 MB of state)",
+                                  "fs_over_fd_time_per_step": step_ms / fd_ms}
+
     if rank == 0 and not args.no_cufft:
         line["cufft_side_reference"] = cufft_side_reference(torch, n, p, prec, dx, dt, c0, eta0, stream)
 
