@@ -395,7 +395,7 @@ def run_ours(args):
     barrier()
     fd_ms = f0.elapsed_time(f1) / kfd
     fd.close()
-    fd_bytes = 2 * F * R if len(n) == 2 else (3 * p + 5) * R
+    fd_bytes = 2 * F * R                      # fused kernels: every field read once and written once per step
     if concurrent:
         line["concurrent_replicas"] = concurrent
     line["fd_comparison_path"] = {"value": 1e3 / fd_ms, "unit": "steps/s", "us_per_step": 1e3 * fd_ms, "steps": kfd,

@@ -9,7 +9,7 @@
 //       eta_i with a halo of one -- forms mu on the tile plus a ring of one point (kernel (i)), and from that
 //       the new c and eta_i of the tile (kernels (ii), (iii)): each field is read once and written once per step,
 //       2(p+1) R bytes instead of the (3p+5) R of the separate kernels (the halo re-reads stay in L1/L2).
-//   3D: kernels (i) and (ii)+(iii) as two launches on global memory (neighbours served by L1/L2).
+//   3D: ONE launch per step as well: a CTA marches along z with rings of planes in shared memory (fd_fused3d_kernel).
 #include "pf_kernels.cuh"
 
 #ifndef PF_FD_TY
@@ -43,43 +43,6 @@ __device__ __forceinline__ Nbr neighbours(long i, int nx, int ny, int nz)
     n.zm = i + (z == 0 ? (long)(nz - 1) * pl : -pl);
     n.zp = i + (z == nz - 1 ? -(long)(nz - 1) * pl : pl);
     return n;
-}
-
-template <typename T>
-__device__ __forceinline__ T lap(const T *__restrict__ u, long i, const Nbr &n, const T (&rdx2)[3], bool threeD)
-{
-    const T v = u[i];
-    T s = rdx2[0] * (u[n.xp] + u[n.xm] - T(2) * v) + rdx2[1] * (u[n.yp] + u[n.ym] - T(2) * v);
-    if (threeD) s += rdx2[2] * (u[n.zp] + u[n.zm] - T(2) * v);
-    return s;
-}
-
-// kernel (i): mu = df_chem/dc - kappa_c lap c
-template <typename T> __global__ void fd_mu_kernel(const FdParams<T> p)
-{
-    const long i = (long)blockIdx.x * blockDim.x + threadIdx.x;
-    if (i >= p.N) return;
-    const Nbr n = neighbours(i, p.nx, p.ny, p.nz);
-    T h = 0;
-    for (int k = 0; k < p.m.n_eta; ++k) h += h_term(p.eta[(long)k * p.N + i]);
-    p.mu[i] = dfdc(p.m, p.c[i], h) - p.m.kappa_c * lap(p.c, i, n, p.rdx2, p.nz > 1);
-}
-
-// kernels (ii) + (iii)
-template <typename T> __global__ void fd_update_kernel(const FdParams<T> p)
-{
-    const long i = (long)blockIdx.x * blockDim.x + threadIdx.x;
-    if (i >= p.N) return;
-    const bool threeD = p.nz > 1;
-    const Nbr n = neighbours(i, p.nx, p.ny, p.nz);
-    const T c = p.c[i];
-    p.c_new[i] = c + p.m.dtM * lap(p.mu, i, n, p.rdx2, threeD);
-    T s2 = 0;
-    for (int k = 0; k < p.m.n_eta; ++k) { const T e = p.eta[(long)k * p.N + i]; s2 += e * e; }
-    for (int k = 0; k < p.m.n_eta; ++k) {
-        const T *e = p.eta + (long)k * p.N;
-        p.eta_new[(long)k * p.N + i] = e[i] - p.m.dtL * (dfdeta(p.m, c, e[i], s2) - p.m.kappa_eta * lap(e, i, n, p.rdx2, threeD));
-    }
 }
 
 // 2D fused step, see the header. Dynamic shared memory: c tile (TY+4) x (TX+4), mu tile (TY+2) x (TX+2),
@@ -154,6 +117,109 @@ __global__ void __launch_bounds__(256) fd_fused2d_kernel(const FdParams<T> p)
     }
 }
 
+// 3D fused step: a CTA owns a TX x TY tile of (x, y) and marches along z over a chunk of zc planes, keeping in shared
+// memory rings of the last planes it needs: c (halo 2 in x, y; 4 slots), every eta_i (halo 1; 4 slots) and mu (tile +
+// ring of one point; 3 slots). Per output plane k: queue c(k+2), eta(k+1) with cp.async; form mu(k+1) from c(k..k+2) and
+// eta(k+1); then c', eta' of plane k from mu(k-1..k+1), eta(k-1..k+1). Each field is read about once ((1 + halo) x
+// (1 + 4/zc)) and written once per step instead of the (3p+5) R of the two global-memory kernels. Two barriers per plane:
+// the 4-slot rings make the next plane's loads land in slots no thread still reads.
+template <typename T, int TX, int TY, int NE>
+__global__ void __launch_bounds__(TX * TY) fd_fused3d_kernel(const FdParams<T> p, const int zc)
+{
+    constexpr int CW = TX + 4, CH = TY + 4, EW = TX + 2, EH = TY + 2, CP = CW * CH, EP = EW * EH;
+    extern __shared__ __align__(16) unsigned char fd_smem[];
+    T *sc = reinterpret_cast<T *>(fd_smem);          // [4][CP]
+    T *smu = sc + 4 * CP;                            // [3][EP]
+    T *se = smu + 3 * EP;                            // [NE][4][EP]
+    const int x0 = blockIdx.x * TX, y0 = blockIdx.y * TY, z0 = blockIdx.z * zc;
+    const int mx = p.nx - 1, my = p.ny - 1, mz = p.nz - 1;
+    const long plane = (long)p.nx * p.ny;
+    const int tx = threadIdx.x % TX, ty = threadIdx.x / TX;
+
+    auto load_c = [&](int m) {                       // plane z0 + m -> slot m & 3
+        const T *src = p.c + (long)((z0 + m) & mz) * plane;
+        T *dst = sc + ((m + 4) & 3) * CP;
+        for (int ly = ty; ly < CH; ly += TY) {
+            const T *row = src + (long)((y0 + ly - 2) & my) * p.nx;
+            cp_async_elem(dst + ly * CW + tx, row + ((x0 + tx - 2) & mx));
+            if (tx < 4) cp_async_elem(dst + ly * CW + TX + tx, row + ((x0 + TX + tx - 2) & mx));
+        }
+    };
+    auto load_e = [&](int m) {
+        for (int k = 0; k < NE; ++k) {
+            const T *src = p.eta + (long)k * p.N + (long)((z0 + m) & mz) * plane;
+            T *dst = se + (k * 4 + ((m + 4) & 3)) * EP;
+            for (int ly = ty; ly < EH; ly += TY) {
+                const T *row = src + (long)((y0 + ly - 1) & my) * p.nx;
+                cp_async_elem(dst + ly * EW + tx, row + ((x0 + tx - 1) & mx));
+                if (tx < 2) cp_async_elem(dst + ly * EW + TX + tx, row + ((x0 + TX + tx - 1) & mx));
+            }
+        }
+    };
+    // kernel (i) for plane m on the tile and its ring; slot3 = m mod 3 kept by the caller
+    auto mu_plane = [&](int m, int slot3) {
+        const T *c0 = sc + ((m + 4) & 3) * CP, *cm = sc + ((m + 3) & 3) * CP, *cp = sc + ((m + 5) & 3) * CP;
+        T *mu = smu + slot3 * EP;
+        auto at = [&](int lx, int ly) {
+            const int i = ly * EW + lx, ci = (ly + 1) * CW + (lx + 1);
+            const T v = c0[ci];
+            const T l = p.rdx2[0] * (c0[ci + 1] + c0[ci - 1] - T(2) * v) + p.rdx2[1] * (c0[ci + CW] + c0[ci - CW] - T(2) * v)
+                      + p.rdx2[2] * (cp[ci] + cm[ci] - T(2) * v);
+            T h = 0;
+            for (int k = 0; k < NE; ++k) h += h_term(se[(k * 4 + ((m + 4) & 3)) * EP + i]);
+            mu[i] = dfdc(p.m, v, h) - p.m.kappa_c * l;
+        };
+        for (int ly = ty; ly < EH; ly += TY) {
+            at(tx, ly);
+            if (tx < 2) at(TX + tx, ly);
+        }
+    };
+
+    grid_dependency_wait();
+    grid_dependents_launch();
+
+    // prologue: mu(-1) and mu(0)
+    load_c(-2); load_c(-1); load_c(0); load_e(-1); load_e(0);
+    cp_async_wait_all();
+    __syncthreads();
+    mu_plane(-1, 2);
+    load_c(1);                                       // slot of c(-3): free
+    cp_async_wait_all();
+    __syncthreads();
+    mu_plane(0, 0);
+    // no barrier needed here: the loop starts with loads into free slots and a barrier before mu(k+1) is formed
+
+    int s3 = 0;                                      // k mod 3
+    for (int k = 0; k < zc; ++k) {
+        load_c(k + 2);                               // slot of c(k-2)
+        load_e(k + 1);                               // slot of eta(k-3)
+        cp_async_wait_all();
+        __syncthreads();
+        const int s3p = (s3 == 2) ? 0 : s3 + 1, s3m = (s3 == 0) ? 2 : s3 - 1;
+        mu_plane(k + 1, s3p);                        // overwrites mu(k-2)
+        __syncthreads();
+
+        // kernels (ii) + (iii) on plane k
+        const int e0 = (ty + 1) * EW + (tx + 1);
+        const long g = (long)((z0 + k) & mz) * plane + (long)(y0 + ty) * p.nx + (x0 + tx);
+        const T c = sc[((k + 4) & 3) * CP + (ty + 2) * CW + (tx + 2)];
+        const T *mu = smu + s3 * EP + e0;
+        const T lm = p.rdx2[0] * (mu[1] + mu[-1] - T(2) * mu[0]) + p.rdx2[1] * (mu[EW] + mu[-EW] - T(2) * mu[0])
+                   + p.rdx2[2] * (smu[s3p * EP + e0] + smu[s3m * EP + e0] - T(2) * mu[0]);
+        p.c_new[g] = c + p.m.dtM * lm;
+        T s2 = 0;
+        for (int f = 0; f < NE; ++f) { const T e = se[(f * 4 + ((k + 4) & 3)) * EP + e0]; s2 += e * e; }
+        for (int f = 0; f < NE; ++f) {
+            const T *e = se + (f * 4 + ((k + 4) & 3)) * EP + e0;
+            const T ezp = se[(f * 4 + ((k + 5) & 3)) * EP + e0], ezm = se[(f * 4 + ((k + 3) & 3)) * EP + e0];
+            const T le = p.rdx2[0] * (e[1] + e[-1] - T(2) * e[0]) + p.rdx2[1] * (e[EW] + e[-EW] - T(2) * e[0])
+                       + p.rdx2[2] * (ezp + ezm - T(2) * e[0]);
+            p.eta_new[(long)f * p.N + g] = e[0] - p.m.dtL * (dfdeta(p.m, c, e[0], s2) - p.m.kappa_eta * le);
+        }
+        s3 = s3p;
+    }
+}
+
 // Eq. 1 pieces in real space: acc[0] += sum f_chem, acc[1] += sum |grad c|^2, acc[2+i] += sum |grad eta_i|^2
 // (forward differences when gradient_kind == 1). Accumulated in fp64; scaled by the caller.
 template <typename T> __global__ void energy_kernel(const EnergyParams<T> p)
@@ -200,16 +266,6 @@ template <typename T> __global__ void energy_kernel(const EnergyParams<T> p)
     }
 }
 
-template <typename T> cudaError_t launch_fd_mu(const FdParams<T> &p, cudaStream_t s)
-{
-    fd_mu_kernel<T><<<(unsigned)((p.N + 255) / 256), 256, 0, s>>>(p);
-    return cudaGetLastError();
-}
-template <typename T> cudaError_t launch_fd_update(const FdParams<T> &p, cudaStream_t s)
-{
-    fd_update_kernel<T><<<(unsigned)((p.N + 255) / 256), 256, 0, s>>>(p);
-    return cudaGetLastError();
-}
 template <typename T, int TX, int TY, int NE> static cudaError_t launch_fd_fused2d_ne(const FdParams<T> &p, cudaStream_t s)
 {
     const size_t smem = sizeof(T) * ((size_t)(TX + 4) * (TY + 4) + (size_t)(1 + NE) * (TX + 2) * (TY + 2));
@@ -244,6 +300,42 @@ template <typename T> cudaError_t launch_fd_fused2d(const FdParams<T> &p, cudaSt
     if (p.nx >= 32) return launch_fd_fused2d_inst<T, 32, PF_FD_TY>(p, s);
     return launch_fd_fused2d_inst<T, 16, 16>(p, s);
 }
+template <typename T, int TX, int TY, int NE> static cudaError_t launch_fd_fused3d_ne(const FdParams<T> &p, cudaStream_t s)
+{
+    const size_t smem = sizeof(T) * ((size_t)4 * (TX + 4) * (TY + 4) + (size_t)(3 + 4 * NE) * (TX + 2) * (TY + 2));
+    auto kern = fd_fused3d_kernel<T, TX, TY, NE>;
+    if (smem > 48 * 1024) {
+        cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        if (e != cudaSuccess) return e;
+    }
+    // chunks along z: enough CTAs for ~8 per SM, at least 16 planes per chunk (4 extra planes are read per chunk)
+    const int tiles = (p.nx / TX) * (p.ny / TY);
+    int chunks = 1;
+    while (tiles * chunks < 1184 && p.nz / (2 * chunks) >= 16) chunks *= 2;
+    const int zc = p.nz / chunks;
+    return launch_pdl(kern, dim3((unsigned)(p.nx / TX), (unsigned)(p.ny / TY), (unsigned)chunks), dim3(TX * TY), smem, s, true, p, zc);
+}
+template <typename T, int TX, int TY> static cudaError_t launch_fd_fused3d_inst(const FdParams<T> &p, cudaStream_t s)
+{
+    switch (p.m.n_eta) {
+    case 0: return launch_fd_fused3d_ne<T, TX, TY, 0>(p, s);
+    case 1: return launch_fd_fused3d_ne<T, TX, TY, 1>(p, s);
+    case 2: return launch_fd_fused3d_ne<T, TX, TY, 2>(p, s);
+    case 3: return launch_fd_fused3d_ne<T, TX, TY, 3>(p, s);
+    case 4: return launch_fd_fused3d_ne<T, TX, TY, 4>(p, s);
+    case 5: return launch_fd_fused3d_ne<T, TX, TY, 5>(p, s);
+    case 6: return launch_fd_fused3d_ne<T, TX, TY, 6>(p, s);
+    case 7: return launch_fd_fused3d_ne<T, TX, TY, 7>(p, s);
+    case 8: return launch_fd_fused3d_ne<T, TX, TY, 8>(p, s);
+    }
+    return cudaErrorInvalidValue;
+}
+// one fused launch per 3D step
+template <typename T> cudaError_t launch_fd_fused3d(const FdParams<T> &p, cudaStream_t s)
+{
+    if (p.nx >= 32) return launch_fd_fused3d_inst<T, 32, 8>(p, s);
+    return launch_fd_fused3d_inst<T, 16, 16>(p, s);
+}
 template <typename T> cudaError_t launch_energy(const EnergyParams<T> &p, cudaStream_t s)
 {
     long blocks = (p.N + 255) / 256;
@@ -252,10 +344,8 @@ template <typename T> cudaError_t launch_energy(const EnergyParams<T> &p, cudaSt
     return cudaGetLastError();
 }
 
-template cudaError_t launch_fd_mu<double>(const FdParams<double> &, cudaStream_t);
-template cudaError_t launch_fd_mu<float>(const FdParams<float> &, cudaStream_t);
-template cudaError_t launch_fd_update<double>(const FdParams<double> &, cudaStream_t);
-template cudaError_t launch_fd_update<float>(const FdParams<float> &, cudaStream_t);
+template cudaError_t launch_fd_fused3d<double>(const FdParams<double> &, cudaStream_t);
+template cudaError_t launch_fd_fused3d<float>(const FdParams<float> &, cudaStream_t);
 template cudaError_t launch_fd_fused2d<double>(const FdParams<double> &, cudaStream_t);
 template cudaError_t launch_fd_fused2d<float>(const FdParams<float> &, cudaStream_t);
 template cudaError_t launch_energy<double>(const EnergyParams<double> &, cudaStream_t);

@@ -8,7 +8,6 @@
 //   s2       [F][nz][ny][P2] complex, 3D only: (kx,ky)-spectral, z-real planes; s2[0] carries c between steps
 //   g2       [nz][ny][P2]   complex, 3D only
 //   park     [nz][ny][P2+16] complex scratch of the column kernels (dt M |xi|^2 g^ of the Cahn-Hilliard update)
-//   mu       [N]            FD chemical potential
 //   tables   twiddles exp(-2 pi i k/n) for M, ny, nz, nx; |xi_d|^2 per axis (Eq. 16-21)
 #include <cmath>
 #include <cstdio>
@@ -40,7 +39,7 @@ struct pf_ctx {
     bool graph_ok = true;
     void *real[2] = {nullptr, nullptr};
     int cur = 0;
-    void *zst = nullptr, *zg = nullptr, *s2 = nullptr, *g2 = nullptr, *mu = nullptr, *park = nullptr;
+    void *zst = nullptr, *zg = nullptr, *s2 = nullptr, *g2 = nullptr, *park = nullptr;
     void *tw_m = nullptr, *tw_y = nullptr, *tw_z = nullptr, *tw_nx = nullptr;
     void *kx2 = nullptr, *ky2 = nullptr, *kz2 = nullptr;
     double *acc = nullptr;
@@ -328,7 +327,6 @@ template <typename T> int step_fd(pf_ctx *c, int nsteps)
     f.nx = c->p.n[0]; f.ny = c->p.n[1]; f.nz = c->p.n[2]; f.N = c->N;
     for (int d = 0; d < 3; ++d) f.rdx2[d] = (d < c->p.ndim) ? (T)(1.0 / (c->p.dx[d] * c->p.dx[d])) : (T)0;
     f.m = make_model<T>(c->p);
-    f.mu = (T *)c->mu;
     for (int s = 0; s < nsteps; ++s) {
         T *cu = (T *)c->real[c->cur], *nw = (T *)c->real[c->cur ^ 1];
         f.c = cu; f.eta = cu + c->N; f.c_new = nw; f.eta_new = nw + c->N;
@@ -336,9 +334,8 @@ template <typename T> int step_fd(pf_ctx *c, int nsteps)
             PF_CK(c, launch_fd_fused2d<T>(f, c->stream));
             c->launches += 1;
         } else {
-            PF_CK(c, launch_fd_mu<T>(f, c->stream));
-            PF_CK(c, launch_fd_update<T>(f, c->stream));
-            c->launches += 2;
+            PF_CK(c, launch_fd_fused3d<T>(f, c->stream));
+            c->launches += 1;
         }
         c->cur ^= 1;
     }
@@ -425,7 +422,7 @@ void pf_destroy(pf_ctx *c)
     if (!c) return;
     drop_graph(c);
     for (auto &e : c->pev) if (e) cudaEventDestroy(e);
-    void *bufs[] = {c->real[0], c->real[1], c->zst, c->zg, c->s2, c->g2, c->mu, c->park, c->tw_m, c->tw_y, c->tw_z,
+    void *bufs[] = {c->real[0], c->real[1], c->zst, c->zg, c->s2, c->g2, c->park, c->tw_m, c->tw_y, c->tw_z,
                     c->tw_nx, c->kx2, c->ky2, c->kz2, c->acc};
     for (void *b : bufs) if (b) cudaFree(b);
     if (c->own_stream) cudaStreamDestroy(c->stream);
@@ -473,7 +470,7 @@ int pf_create(const pf_params *p, pf_ctx **out)
     const size_t fb = (size_t)c->N * c->w;                 // one real field
     int rc;
     if ((rc = alloc(&c->real[0], fb * c->F)) || (rc = alloc(&c->real[1], fb * c->F)) ||
-        (rc = alloc(&c->zst, fb * c->F)) || (rc = alloc(&c->zg, fb)) || (rc = alloc(&c->mu, fb)) ||
+        (rc = alloc(&c->zst, fb * c->F)) || (rc = alloc(&c->zg, fb)) ||
         (rc = alloc((void **)&c->acc, sizeof(double) * 32)) ||
         (rc = alloc(&c->park, (size_t)(c->P2 + 16) * c->p.n[1] * c->p.n[2] * 2 * c->w)))
         return fail(rc);

@@ -71,7 +71,6 @@ template <typename T> struct ColParams {
 // FD path
 template <typename T> struct FdParams {
     const T *c, *eta;        // time-t fields
-    T       *mu;             // chemical potential scratch
     T       *c_new, *eta_new;
     int      nx, ny, nz;
     long     N;              // nx*ny*nz
@@ -92,9 +91,8 @@ template <typename T> struct EnergyParams {
 // ---- launchers (defined in the .cu files; return cudaGetLastError()) ----
 template <typename T> cudaError_t launch_row(int mode, int nx, const RowParams<T> &p, cudaStream_t s);
 template <typename T> cudaError_t launch_col(int mode, int nfft, int nslots, int nbatch, const ColParams<T> &p, cudaStream_t s);
-template <typename T> cudaError_t launch_fd_mu(const FdParams<T> &p, cudaStream_t s);
-template <typename T> cudaError_t launch_fd_update(const FdParams<T> &p, cudaStream_t s);
 template <typename T> cudaError_t launch_fd_fused2d(const FdParams<T> &p, cudaStream_t s);
+template <typename T> cudaError_t launch_fd_fused3d(const FdParams<T> &p, cudaStream_t s);
 template <typename T> cudaError_t launch_energy(const EnergyParams<T> &p, cudaStream_t s);
 
 #if defined(__CUDACC__)
@@ -132,8 +130,8 @@ __device__ __forceinline__ void bulk_load(void *smem_dst, const void *gmem_src, 
                  ::"r"(smem_addr(smem_dst)), "l"(gmem_src), "r"(bytes), "r"(smem_addr(bar)) : "memory");
 }
 
-template <typename K, typename P>
-static inline cudaError_t launch_pdl(K kern, dim3 grid, dim3 block, size_t smem, cudaStream_t s, bool pdl, const P &params)
+template <typename K, typename... P>
+static inline cudaError_t launch_pdl(K kern, dim3 grid, dim3 block, size_t smem, cudaStream_t s, bool pdl, const P &...params)
 {
     cudaLaunchConfig_t cfg = {};
     cfg.gridDim = grid; cfg.blockDim = block; cfg.dynamicSmemBytes = smem; cfg.stream = s;
@@ -141,7 +139,7 @@ static inline cudaError_t launch_pdl(K kern, dim3 grid, dim3 block, size_t smem,
     at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
     at[0].val.programmaticStreamSerializationAllowed = 1;
     cfg.attrs = at; cfg.numAttrs = pdl ? 1 : 0;
-    return cudaLaunchKernelEx(&cfg, kern, params);
+    return cudaLaunchKernelEx(&cfg, kern, params...);
 }
 #endif
 

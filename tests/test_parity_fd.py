@@ -72,3 +72,13 @@ def test_free_energy(oracle, n, kind):
     np.testing.assert_allclose(e1, m.free_energy(rc, reta, kind), rtol=1e-9)
     assert e1[0] < e0[0]                      # monotone decrease
     assert rel_linf([gc, geta], [rc, reta]) < 1e-10
+
+
+@pytest.mark.parametrize("n,n_eta,steps", [((16, 16, 16), 1, 40), ((32, 16, 64), 3, 30), ((64, 64, 64), 2, 20), ((128, 32, 256), 2, 6)])
+def test_fd_fused_3d_planes(oracle, n, n_eta, steps):
+    # the plane-marching 3D kernel: both tile shapes (16 x 16, 32 x 8), one and several z chunks, rings wrapping in z
+    c, eta, dx = make_init("B", n, n_eta)
+    kt2 = sum(4.0 / d ** 2 for d in dx)
+    dt = min(0.75 * 2.0 / (5.0 * kt2 * (4.0 + 3.0 * kt2)), 2e-3)
+    (gc, geta), (rc, reta) = run_both(oracle, n=n, n_eta=n_eta, init="B", steps=steps, dt=dt, method="fd")
+    assert rel_linf([gc, geta], [rc, reta]) < 1e-12
