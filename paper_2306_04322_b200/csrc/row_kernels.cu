@@ -20,6 +20,9 @@
 #include <type_traits>
 #include "pf_kernels.cuh"
 
+#ifndef PF_ROW_THREADS
+#define PF_ROW_THREADS 256
+#endif
 #ifndef PF_ROW_E1024
 #define PF_ROW_E1024 8
 #endif
@@ -150,7 +153,7 @@ static cudaError_t launch_row_inst(const RowParams<T> &p, cudaStream_t s)
     constexpr int TT = M / E;
     const int per_row = TT * p.F;
     if (per_row > 1024) return cudaErrorInvalidConfiguration;
-    int RB = 256 / per_row;
+    int RB = PF_ROW_THREADS / per_row;
     if (RB > p.nrows / 296) RB = p.nrows / 296;      // small grids: at least two CTAs per SM before rows are batched
     if (RB < 1) RB = 1;
     if (RB > p.nrows) RB = p.nrows;
