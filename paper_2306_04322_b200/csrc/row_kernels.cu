@@ -44,7 +44,12 @@ struct CtaSync { __device__ __forceinline__ void operator()() const { __syncthre
 // a transform carried by exactly one warp exchanges through its own buffer: warp-level synchronisation is enough,
 // and the warps of an SM drift apart (their fp64 and shared-memory phases overlap instead of alternating)
 struct WarpSync { __device__ __forceinline__ void operator()() const { __syncwarp(); } };
-template <int TT> struct FftSync { typedef typename std::conditional<(TT <= 32), WarpSync, CtaSync>::type type; };
+// a transform carried by several warps: named barrier over exactly its TT threads (ids 1..15; id 0 is __syncthreads),
+// so the transforms of a CTA (fields, rows) drift apart between the points where the nonlinear terms couple them
+struct GroupSync {
+    int id, n;
+    __device__ __forceinline__ void operator()() const { asm volatile("bar.sync %0, %1;" ::"r"(id), "r"(n) : "memory"); }
+};
 
 
 template <int M, int E> __host__ __device__ constexpr int row_pitch() { return M + (M >> 3) + 1; }
@@ -75,7 +80,7 @@ __global__ void __maxnreg__(PF_ROW_REGS(M, E)) row_kernel(const RowParams<T> p)
     const bool valid = row < p.nrows;
     RowBuf<C, 3> buf{smem + (long)rf * MP};
     const CtaSync sync;
-    const typename FftSync<TT>::type fsync;
+    const int rf_sync = threadIdx.x / TT;              // transform index within the CTA (at most 9 when TT > 32)
 
     grid_dependency_wait();
     grid_dependents_launch();
@@ -89,7 +94,8 @@ __global__ void __maxnreg__(PF_ROW_REGS(M, E)) row_kernel(const RowParams<T> p)
         const C *src = p.zst + f * p.zfs + row * M;
 #pragma unroll
         for (int q = 0; q < E; ++q) v[q] = valid ? cswap(src[j + q * TT]) : mk<T>(0, 0);   // swap: inverse via forward
-        fft_forward<M, E>(v, j, p.tw, buf, fsync);
+        if constexpr (TT <= 32) fft_forward<M, E>(v, j, p.tw, buf, WarpSync());
+        else fft_forward<M, E>(v, j, p.tw, buf, GroupSync{1 + rf_sync, TT});
         const T s = T(1) / T(M);
 #pragma unroll
         for (int q = 0; q < E; ++q) v[q] = mk<T>(v[q].y * s, v[q].x * s);                    // swap back, normalise
@@ -136,8 +142,9 @@ __global__ void __maxnreg__(PF_ROW_REGS(M, E)) row_kernel(const RowParams<T> p)
     }
 
     // with warp-level exchange barriers the buffers the other fields' threads have just read need a CTA barrier
-    if (MODE == ROW_STEP && TT <= 32) sync();
-    fft_forward<M, E>(v, j, p.tw, buf, fsync);
+    if (MODE == ROW_STEP) sync();
+    if constexpr (TT <= 32) fft_forward<M, E>(v, j, p.tw, buf, WarpSync());
+    else fft_forward<M, E>(v, j, p.tw, buf, GroupSync{1 + rf_sync, TT});
 
     C *dst = (MODE == ROW_STEP && f == 0) ? (p.zg + row * M) : (p.zst + f * p.zfs + row * M);
     if (valid) {
