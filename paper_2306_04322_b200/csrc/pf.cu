@@ -516,16 +516,16 @@ int pf_get_fields(pf_ctx *c, void *fc, void *eta, int where)
 int pf_step_fs(pf_ctx *c, int nsteps)
 {
     if (!c || nsteps < 0) return PF_EINVAL;
-    if (c->state == ST_NONE) return PF_ESTATE;
     if (nsteps == 0) return PF_OK;
+    if (c->state == ST_NONE) return PF_ESTATE;
     return (c->p.precision == PF_F64) ? step_fs<double>(c, nsteps) : step_fs<float>(c, nsteps);
 }
 
 int pf_step_fd(pf_ctx *c, int nsteps)
 {
     if (!c || nsteps < 0) return PF_EINVAL;
-    if (c->state == ST_NONE) return PF_ESTATE;
     if (nsteps == 0) return PF_OK;
+    if (c->state == ST_NONE) return PF_ESTATE;
     return (c->p.precision == PF_F64) ? step_fd<double>(c, nsteps) : step_fd<float>(c, nsteps);
 }
 
