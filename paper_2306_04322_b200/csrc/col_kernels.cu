@@ -41,6 +41,12 @@
 #ifndef PF_TP_512
 #define PF_TP_512 2
 #endif
+#ifndef PF_F32_TP_1024
+#define PF_F32_TP_1024 4
+#endif
+#ifndef PF_F32_TP_2048
+#define PF_F32_TP_2048 2
+#endif
 #ifndef PF_TP_2048
 #define PF_TP_2048 2
 #endif
@@ -290,6 +296,13 @@ static cudaError_t launch_col_mode(int mode, int nslots, int nbatch, const ColPa
 // two exchange buffers of a CTA within 128 KB for long ones.
 template <typename T> cudaError_t launch_col(int mode, int nfft, int nslots, int nbatch, const ColParams<T> &p, cudaStream_t s)
 {
+    // fp32: 16 elements per thread (the bytes an fp64 thread holds with 8) and twice the column pairs per CTA (32-byte pieces)
+    if (sizeof(T) == 4) {
+        switch (nfft) {
+        case 1024: return launch_col_mode<T, 1024, 16, PF_F32_TP_1024>(mode, nslots, nbatch, p, s);
+        case 2048: return launch_col_mode<T, 2048, 16, PF_F32_TP_2048>(mode, nslots, nbatch, p, s);
+        }
+    }
     switch (nfft) {
 #ifndef PF_ONLY_N
     case 16:   return launch_col_mode<T, 16, 8, 8>(mode, nslots, nbatch, p, s);

@@ -29,7 +29,7 @@
 #ifndef PF_ROW_REGS_BIG
 #define PF_ROW_REGS_BIG 80
 #endif
-#define PF_ROW_REGS(M, E) (((E) >= 16) ? 128 : ((M) >= 256) ? PF_ROW_REGS_BIG : 64)
+#define PF_ROW_REGS(T, M, E) ((((E) >= 16) && sizeof(T) == 8) ? 128 : ((M) >= 256) ? PF_ROW_REGS_BIG : 64)
 
 namespace pf {
 
@@ -58,7 +58,7 @@ template <int M, int E> __host__ __device__ constexpr int row_pitch() { return M
 // than the last few registers (measured on B200: 94 -> 80 registers: 1024^2 row kernel 28.1 -> 26.4 us; 64 at
 // nx = 256: 394 -> 317 us at 256^3).
 template <typename T, int M, int E, int MODE>
-__global__ void __maxnreg__(PF_ROW_REGS(M, E)) row_kernel(const RowParams<T> p)
+__global__ void __maxnreg__(PF_ROW_REGS(T, M, E)) row_kernel(const RowParams<T> p)
 {
 #ifdef PF_DBG_EMPTY
     return;
@@ -196,7 +196,8 @@ template <typename T> cudaError_t launch_row(int mode, int nx, const RowParams<T
     case 128:  return launch_row_mode<T, 128, 8>(mode, p, s);
     case 256:  return launch_row_mode<T, 256, 8>(mode, p, s);
     case 512:  return launch_row_mode<T, 512, 8>(mode, p, s);
-    case 1024: return launch_row_mode<T, 1024, PF_ROW_E1024>(mode, p, s);
+    // fp32 at nx = 2048: 16 elements per thread (the bytes an fp64 thread holds with 8), two CTAs per SM
+    case 1024: return (sizeof(T) == 4) ? launch_row_mode<T, 1024, 16>(mode, p, s) : launch_row_mode<T, 1024, PF_ROW_E1024>(mode, p, s);
     }
     return cudaErrorInvalidValue;
 }

@@ -100,6 +100,7 @@ int main()
     shape<double, 2048, 8, 1>(); shape<double, 1024, 16, 2>();
     shape<float, 16, 8, 8>(); shape<float, 64, 8, 4>(); shape<float, 256, 8, 4>(); shape<float, 512, 8, 2>();
     shape<float, 1024, 8, 2>(); shape<float, 2048, 8, 2>(); shape<float, 2048, 8, 1>();
+    shape<float, 1024, 16, 4>(); shape<float, 2048, 16, 2>(); shape<float, 2048, 16, 4>();
     if (fails) { printf("%d FAILURES\n", fails); return 1; }
     printf("ALL OK\n");
     return 0;
