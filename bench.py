@@ -334,8 +334,43 @@ def run_ours(args):
     torch.cuda.synchronize()
     e2e_s = time.perf_counter() - t0
     e2e_s = replicas.max_over_ranks(e2e_s, device="cuda")
-    e2e = {"value": world * ke / e2e_s, "unit": "steps/s", "h2d_bytes_per_step": F * R, "d2h_bytes_per_step": F * R,
-           "steps": ke, "note": "pf_set_fields(HOST) + pf_step_fs(1) + pf_get_fields(HOST) per step, pinned host buffers"}
+    serial_e2e = world * ke / e2e_s
+    # the same loop for two independent simulations from two host threads (own context, stream and pinned buffers
+    # each): the H2D copy of one overlaps the D2H copy of the other (PCIe is full duplex)
+    import threading
+    cxs2 = [pf.Context(n, n_eta=p, dx=dx, dt=dt, precision=prec) for _ in range(2)]
+    bufs2 = []
+    for _ in range(2):
+        bc = torch.empty(tuple(reversed(n)), dtype=tdt).pin_memory()
+        be = torch.empty((p,) + tuple(reversed(n)), dtype=tdt).pin_memory()
+        bc.numpy()[...] = c0
+        be.numpy()[...] = eta0
+        bufs2.append((bc, be))
+
+    def worker(i, steps):
+        h, (bc, be) = cxs2[i]._h, bufs2[i]
+        for _ in range(steps):
+            L.pf_set_fields(h, bc.data_ptr(), be.data_ptr(), pf.PF_HOST)
+            L.pf_step_fs(h, 1)
+            L.pf_get_fields(h, bc.data_ptr(), be.data_ptr(), pf.PF_HOST)
+
+    for i in range(2):
+        worker(i, 2)
+    barrier()
+    t0 = time.perf_counter()
+    th = [threading.Thread(target=worker, args=(i, ke)) for i in range(2)]
+    for t in th:
+        t.start()
+    for t in th:
+        t.join()
+    torch.cuda.synchronize()
+    e2e2_s = replicas.max_over_ranks(time.perf_counter() - t0, device="cuda")
+    for cx2 in cxs2:
+        cx2.close()
+    e2e = {"value": world * 2 * ke / e2e2_s, "unit": "steps/s", "h2d_bytes_per_step": F * R, "d2h_bytes_per_step": F * R,
+           "steps": 2 * ke, "contexts": 2, "one_context_value": serial_e2e,
+           "note": "pf_set_fields(HOST) + pf_step_fs(1) + pf_get_fields(HOST) per step, pinned host buffers; two independent "
+                   "simulations driven from two host threads so that uploads and downloads overlap; one_context_value = the same loop for one simulation"}
 
     line = {"metric": METRIC, "value": value, "unit": "steps/s", "n_gpus": world, "steps": K, "warmup": W,
             "ms_per_step": step_ms, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": prec,
