@@ -90,6 +90,12 @@ def test_c3_2048_sq_p4(oracle):
     _check(oracle, TOL32, n=(2048, 2048), n_eta=4, init="B", steps=3, dt=5e-3, precision="f32")
 
 
+def test_fp32_1024_sq_wide_column_blocks(oracle):
+    # fp32 at ny = 1024 uses its own strided-kernel shape (16 elements per thread, four column pairs per CTA)
+    _check(oracle, TOL32, n=(1024, 1024), n_eta=2, init="B", steps=5, dt=5e-3, precision="f32")
+    _check(oracle, TOL32, n=(64, 1024), n_eta=1, init="B", steps=5, dt=5e-3, precision="f32")
+
+
 def test_long_axes_2048(oracle):
     _check(oracle, TOL64, n=(2048, 32), n_eta=1, init="B", steps=10, dt=5e-3)
     _check(oracle, TOL64, n=(32, 2048), n_eta=1, init="B", steps=10, dt=5e-3)
