@@ -1,0 +1,101 @@
+"""The paper's accuracy study on B200 (section 3.3, Fig. 6, Eq. 22).
+
+    python -m paper_2306_04322_b200.accuracy [--grids 128 256 512 1024] [--ref-grid 2048] [--ref-dt 1e-4]
+                                             [--t-end 100] [--fd-max-steps 5e6] [--out results.json]
+
+Benchmark of the paper: l = 200, c + 4 order parameters, initial condition Eqs. 4-5 evolved from
+t = 1 to t = 100. The paper first evolves the (non-periodic) Eq. 5 field from t = 0 to t = 1 with FD "on a fine spatial
+grid and small time step" without giving either; the stand-in here is the semi-implicit Fourier-spectral
+step on the reference grid at the reference time step. The t = 1 field is then sampled on every coarser grid (the grids
+nest) and advanced to t_end with
+  * FS (Eq. 16), FS-FD O(dl^2) (Eq. 17) and FS-FD O(dl^4) (Eq. 18) at dt = 5e-3 and 1e-3 (Table 1),
+  * explicit FD at 0.75 x its linear stability limit (the paper's own steps are 0.72-0.79 of it), capped at 2e-3 where the
+    Allen-Cahn reaction term is the limit; skipped where it would need more than --fd-max-steps steps,
+and compared with the reference (FS on the reference grid at the reference dt) through Eq. 22,
+E_phi = sum (phi - phi_ref)^2 / sum phi_ref^2 with phi = c and phi = sum_i eta_i, printed in percent as in the paper.
+The paper prints two values to compare with: E_c = 2.03 %, E_eta = 7.74 % for FD and FS-FD O(dl^2) on 128^2.
+Everything runs through the C ABI (pf.Context); numpy only samples and compares.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import time
+
+import numpy as np
+
+
+def eq22_percent(phi, ref):
+    return 100.0 * float(np.sum((phi - ref) ** 2) / np.sum(ref ** 2))
+
+
+def advance(pf, n, p, dx, dt, t_span, c, eta, method="fs", k2_kind=0):
+    """Returns (c, eta, steps, seconds) after advancing by t_span with a whole number of steps of size ~dt."""
+    steps = max(1, int(round(t_span / dt)))
+    dt = t_span / steps
+    with pf.Context((n, n), n_eta=p, dx=(dx, dx), dt=dt, k2_kind=k2_kind) as ctx:
+        ctx.set_fields(c, eta)
+        t0 = time.perf_counter()
+        done = 0
+        while done < steps:                      # chunks keep the launch queue short
+            k = min(20000, steps - done)
+            (ctx.step_fs if method == "fs" else ctx.step_fd)(k)
+            done += k
+        out_c, out_eta = ctx.get_fields()
+        return out_c, out_eta, steps, time.perf_counter() - t0
+
+
+def main():
+    from . import pf, synth
+
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--grids", type=int, nargs="+", default=[128, 256, 512, 1024])
+    ap.add_argument("--ref-grid", type=int, default=2048)
+    ap.add_argument("--ref-dt", type=float, default=1e-4)
+    ap.add_argument("--t-end", type=float, default=100.0)
+    ap.add_argument("--fd-max-steps", type=float, default=5e6)
+    ap.add_argument("--out", default=None)
+    a = ap.parse_args()
+    p, length = 4, 200.0
+    M, kc, rho2 = 5.0, 3.0, 2.0
+    nr = a.ref_grid
+    c0, eta0, dx0 = synth.init_b((nr, nr), p)
+    assert abs(dx0[0] - length / nr) < 1e-12
+    # stand-in for the paper's pre-evolution, then the reference run
+    c1, eta1, s, sec = advance(pf, nr, p, length / nr, a.ref_dt, 1.0, c0, eta0)
+    print(f"pre-evolution t=0..1 on {nr}^2, dt={a.ref_dt:g}: {s} FS steps in {sec:.1f} s", flush=True)
+    cr, er, s, sec = advance(pf, nr, p, length / nr, a.ref_dt, a.t_end - 1.0, c1, eta1)
+    print(f"reference     t=1..{a.t_end:g} on {nr}^2, dt={a.ref_dt:g}: {s} FS steps in {sec:.1f} s "
+          f"(finite: {bool(np.isfinite(cr).all())})", flush=True)
+    rows = []
+    print(f"{'grid':>6} {'method':>14} {'dt':>10} {'steps':>9} {'seconds':>8} {'E_c %':>11} {'E_eta %':>11}")
+    for n in a.grids:
+        r = nr // n
+        dx = length / n
+        ci, ei = np.ascontiguousarray(c1[::r, ::r]), np.ascontiguousarray(eta1[:, ::r, ::r])
+        rc, rs = cr[::r, ::r], er.sum(0)[::r, ::r]
+        k2max = 8.0 / dx ** 2
+        dt_fd = min(0.75 * 2.0 / (M * k2max * (2 * rho2 + kc * k2max)), 2e-3)
+        runs = [("FS", "fs", 0, 5e-3), ("FS-FD O(dl^2)", "fs", 1, 5e-3), ("FS-FD O(dl^4)", "fs", 2, 5e-3),
+                ("FS", "fs", 0, 1e-3), ("FS-FD O(dl^2)", "fs", 1, 1e-3), ("FS-FD O(dl^4)", "fs", 2, 1e-3),
+                ("FD", "fd", 0, dt_fd)]
+        for name, method, kind, dt in runs:
+            if method == "fd" and (a.t_end - 1.0) / dt > a.fd_max_steps:
+                print(f"{n:>6} {name:>14} {dt:>10.3e}   skipped: {(a.t_end - 1.0) / dt:.2e} steps", flush=True)
+                continue
+            gc, ge, steps, sec = advance(pf, n, p, dx, dt, a.t_end - 1.0, ci, ei, method, kind)
+            fin = bool(np.isfinite(gc).all() and np.isfinite(ge).all())
+            row = {"grid": n, "method": name, "dt": dt, "steps": steps, "seconds": sec, "finite": fin,
+                   "E_c_percent": eq22_percent(gc, rc) if fin else None,
+                   "E_eta_percent": eq22_percent(ge.sum(0), rs) if fin else None}
+            rows.append(row)
+            ec = f"{row['E_c_percent']:.4e}" if fin else "non-finite"
+            ee = f"{row['E_eta_percent']:.4e}" if fin else "non-finite"
+            print(f"{n:>6} {name:>14} {dt:>10.3e} {steps:>9d} {sec:>8.2f} {ec:>11} {ee:>11}", flush=True)
+    if a.out:
+        with open(a.out, "w") as fh:
+            json.dump({"ref_grid": nr, "ref_dt": a.ref_dt, "t_end": a.t_end, "runs": rows}, fh, indent=1)
+
+
+if __name__ == "__main__":
+    main()

@@ -47,6 +47,9 @@
 #ifndef PF_F32_TP_2048
 #define PF_F32_TP_2048 2
 #endif
+#ifndef PF_TP_1024
+#define PF_TP_1024 2
+#endif
 #ifndef PF_TP_2048
 #define PF_TP_2048 2
 #endif
@@ -313,7 +316,7 @@ template <typename T> cudaError_t launch_col(int mode, int nfft, int nslots, int
     case 512:  return launch_col_mode<T, 512, 8, PF_TP_512>(mode, nslots, nbatch, p, s);
 #endif
 #if !defined(PF_ONLY_N) || PF_ONLY_N == 1024
-    case 1024: return launch_col_mode<T, 1024, 8, 2>(mode, nslots, nbatch, p, s);
+    case 1024: return launch_col_mode<T, 1024, 8, PF_TP_1024>(mode, nslots, nbatch, p, s);
 #endif
 #ifndef PF_ONLY_N
     case 2048: return launch_col_mode<T, 2048, 8, PF_TP_2048>(mode, nslots, nbatch, p, s);
