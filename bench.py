@@ -303,7 +303,7 @@ def run_ours(args):
                 "algorithmic_bytes_note": "SURVEY 8(d) per-pass bytes of the passes this kernel fuses (see DESIGN.md section 5)",
                 "design_bytes_per_launch": kdesign[dom],
                 "achieved_vs_design_bytes": kdesign[dom] / (kms[dom] * 1e-3) / 1e9,
-                "kernel_ms": kms[dom], "kernels_ms": kms, "kernel_timing": f"events around {PROF_REPEAT} back-to-back launches",
+                "kernel_ms": kms[dom], "kernels_ms": kms, "kernel_timing": f"events around {PROF_REPEAT} back-to-back launches of one kernel on one replica (L2 warm after the first; the step time above is the cold-L2 figure)",
                 "kernel_share_of_step": kms[dom] / sum(kms.values())}
     step_ms = ms / K
     step_roofline = {"bytes_per_step_survey_8d": survey_bytes, "bytes_per_step_this_design": design_bytes,
