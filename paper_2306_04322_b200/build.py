@@ -1,6 +1,8 @@
 """Builds libpf.so (the C-ABI library of include/pf.h) in-tree with nvcc for sm_100a.
 
     python -m paper_2306_04322_b200.build [--force]
+    PF_EXTRA_NVCC_FLAGS="-DPF_DBG_SKIP_COMPUTE" PF_BUILD_SUFFIX=nocomp python -m paper_2306_04322_b200.build
+        -> libpf_nocomp.so beside libpf.so (an ablation / experiment build; load it with PF_LIBPF=<path>, see pf.py)
 
 The four translation units are compiled in parallel and linked into
 paper_2306_04322_b200/libpf.so (static cudart; no torch, no other dependency).
@@ -14,13 +16,14 @@ from concurrent.futures import ThreadPoolExecutor
 
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
-OBJ = os.path.join(HERE, "csrc", "build")
-SO = os.path.join(HERE, "libpf.so")
+SUFFIX = os.environ.get("PF_BUILD_SUFFIX", "")
+OBJ = os.path.join(HERE, "csrc", "build" + ("_" + SUFFIX if SUFFIX else ""))
+SO = os.path.join(HERE, "libpf" + ("_" + SUFFIX if SUFFIX else "") + ".so")
 UNITS = ["row_kernels", "col_kernels", "fd_kernels", "pf"]
 HEADERS = [os.path.join(CSRC, h) for h in ("fft_core.cuh", "pf_kernels.cuh")] + \
           [os.path.join(os.path.dirname(HERE), "include", "pf.h")]
 NVCC_FLAGS = ["-std=c++17", "-O3", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo",
-              "-Xcompiler", "-fPIC", "-Xptxas", "-v"]
+              "-Xcompiler", "-fPIC", "-Xptxas", "-v"] + os.environ.get("PF_EXTRA_NVCC_FLAGS", "").split()
 
 
 def _nvcc() -> str:
