@@ -26,6 +26,9 @@
 #include "col_buf.cuh"
 
 // column pairs per CTA at the longer axes (tuned on B200)
+#ifndef PF_COL_THREADS_PER_SM
+#define PF_COL_THREADS_PER_SM 1024
+#endif
 #ifndef PF_TP_32
 #define PF_TP_32 8
 #endif
@@ -74,7 +77,8 @@ template <int N, int E, int TP> struct ColShape {
     static constexpr int TT = N / E;
     static constexpr int SLOTS = 2 * TP;
     static constexpr int THREADS = SLOTS * TT;                           // whole warps
-    static constexpr int MINB = (THREADS >= 1024) ? 1 : ((1024 / THREADS > 32) ? 32 : 1024 / THREADS);   // 64 registers
+    static constexpr int BUDGET = PF_COL_THREADS_PER_SM;                 // resident threads per SM the register cap is set for (1024: 64 registers)
+    static constexpr int MINB = (THREADS >= BUDGET) ? 1 : ((BUDGET / THREADS > 32) ? 32 : BUDGET / THREADS);
     static constexpr int LR = (E >= 16) ? 4 : 3;                         // log2 of the first-stage radix
 };
 
