@@ -87,10 +87,10 @@ def bytes_model(n, p, w):
 # summarised under profiles/ (key: workload -> kernel -> bytes)
 NCU_TRAFFIC = {
     # profiles/r1_ncu_full_1024sq.md (the L2 keeps part of what the previous kernel wrote: traffic < algorithmic bytes)
-    "1024sq": {"row_c2r_nonlinear_r2c": 25220096, "col_y_fft_update_ifft": 33624320 + 91648},
+    "1024sq": {"row_c2r_nonlinear_r2c": 25221120 + 512, "col_y_fft_update_ifft": 33624320 + 27136},
     # profiles/r1_ncu_full_256cube.md
-    "256cube": {"row_c2r_nonlinear_r2c": 402713856 + 354714880, "col_y_fwd": 408621312 + 364992512,
-                "col_z_fft_update_ifft": 604080896 + 544414976, "col_y_inv": 427850240 + 358247168},
+    "256cube": {"row_c2r_nonlinear_r2c": 402713856 + 353691904, "col_y_fwd": 408681216 + 364982528,
+                "col_z_fft_update_ifft": 604053248 + 545553920, "col_y_inv": 427836160 + 358318336},
 }
 
 
