@@ -1,22 +1,27 @@
 #!/usr/bin/env python
 """bench.py -- throughput of the Fourier-spectral (FS) step of arXiv 2306.04322 on B200.
 
-    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload 1024sq|256cube|2048sq|2048sq_f32|512sq|256sq|64sq]
-                    [--impl ours|reference]
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload NAME] [--also NAME ...] [--impl ours|reference]
 
 A "step" is one FS time step (all kernels of SURVEY 8(a): x-pass with the nonlinear evaluation, strided passes with
 the spectral update) of one simulation. At the L2-resident sizes the timed loop cycles through R independent
 replicas of the simulation so that consecutive steps never find their inputs in L2 (timing rule "inputs larger than
-L2"); the single-simulation (L2-resident) figure is reported next to it. Prints ONE JSON line.
+L2"). The timed region of K steps is repeated B >= 5 times; `value` is the median batch.
+Prints ONE JSON line: the headline workload (1024sq, the metric's 2D size) at the top level and the metric's other
+size (256cube) measured in the same invocation under "workloads".
+
+--gpus N > 1 outside torchrun re-executes itself under torch.distributed.run with N ranks (replicas only, no
+data-path collective).
 """
 from __future__ import annotations
 
 import argparse
+import hashlib
 import json
 import os
 import subprocess
 import sys
-import tempfile
+import threading
 import time
 
 import numpy as np
@@ -32,11 +37,15 @@ WORKLOADS = {
     "2048sq_f32": ((2048, 2048), 4, "f32", "B", 5e-3, "2D 2048x2048, c + 4 eta, fp32 (configs[2])"),
     "512sq": ((512, 512), 4, "f64", "B", 5e-3, "2D 512x512, c + 4 eta, fp64 (configs[1] grid)"),
     "256sq": ((256, 256), 4, "f64", "B", 5e-3, "2D 256x256, c + 4 eta, fp64 (paper Table 1 grid; its FS run of PAPER.md:286)"),
+    "128sq": ((128, 128), 4, "f64", "B", 5e-3, "2D 128x128, c + 4 eta, fp64 (paper Table 1 grid)"),
     "64sq": ((64, 64), 2, "f64", "A", 0.05, "2D 64x64, c + 2 eta, fp64 (configs[0])"),
+    "128cube": ((128, 128, 128), 2, "f64", "B", 5e-3, "3D 128^3, c + 2 eta, fp64 (paper Table 2 grid)"),
+    "64cube": ((64, 64, 64), 2, "f64", "B", 5e-3, "3D 64^3, c + 2 eta, fp64 (paper Table 2 grid)"),
 }
-DEFAULT_STEPS = {"1024sq": 20000, "256cube": 1500, "2048sq": 3000, "2048sq_f32": 5000, "512sq": 40000, "256sq": 60000, "64sq": 100000}
+# steps per timed batch when --steps is not given (>= 200); the batch is repeated >= 5 times
+DEFAULT_STEPS = {"1024sq": 2000, "256cube": 200, "2048sq": 400, "2048sq_f32": 600, "512sq": 4000, "256sq": 6000, "128sq": 8000,
+                 "64sq": 10000, "128cube": 1000, "64cube": 4000}
 L2_BYTES = 126e6
-PROF_REPEAT = 8
 METRIC = "FS steps/s (Gpoint-updates/s and achieved HBM GB/s alongside)"
 
 
@@ -83,60 +92,154 @@ def bytes_model(n, p, w):
     return survey, design
 
 
-# dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel, from the ncu --set full captures
-# summarised under profiles/ (key: workload -> kernel -> bytes)
-NCU_TRAFFIC = {
-    # profiles/r1_ncu_full_1024sq.md (the L2 keeps part of what the previous kernel wrote: traffic < algorithmic bytes)
-    "1024sq": {"row_c2r_nonlinear_r2c": 25221120 + 512, "col_y_fft_update_ifft": 33624320 + 27136},
-    # profiles/r1_ncu_full_256cube.md
-    "256cube": {"row_c2r_nonlinear_r2c": 402713856 + 353691904, "col_y_fwd": 408681216 + 364982528,
-                "col_z_fft_update_ifft": 604053248 + 545553920, "col_y_inv": 427836160 + 358318336},
-}
+def kernel_source_hash():
+    """Hash of the kernel sources: the ncu traffic figures under profiles/ are only quoted for the build they were taken from."""
+    h = hashlib.sha256()
+    d = os.path.join(ROOT, "paper_2306_04322_b200", "csrc")
+    for f in sorted(os.listdir(d)):
+        if f.endswith((".cu", ".cuh")):
+            h.update(open(os.path.join(d, f), "rb").read())
+    return h.hexdigest()[:16]
+
+
+def ncu_traffic(workload, kernel):
+    """dram__bytes_read.sum + dram__bytes_write.sum per launch from the committed ncu --set full summary
+    (profiles/ncu_traffic.json, written from the capture named in it). None when the kernel sources have changed since."""
+    try:
+        with open(os.path.join(ROOT, "profiles", "ncu_traffic.json")) as fh:
+            t = json.load(fh)
+        if t.get("kernel_source_hash") != kernel_source_hash():
+            return None, f"profiles/ncu_traffic.json was captured from other kernel sources ({t.get('kernel_source_hash')})"
+        return t["traffic"].get(workload, {}).get(kernel), t.get("capture")
+    except Exception as e:
+        return None, f"no profiles/ncu_traffic.json ({type(e).__name__})"
 
 
 class ClockSampler:
-    FIELDS = "clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown," \
-             "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap"
+    """SM clock, power and clock-event reasons sampled through NVML by a host thread every ~2 ms while the timed batches run
+    (a timed region can be as short as 1 ms, far below what `nvidia-smi -lms` resolves), plus one sample taken right
+    after the last batch was queued. Falls back to one-shot nvidia-smi queries when NVML is unavailable."""
 
-    def __init__(self, index):
-        self.tmp = tempfile.NamedTemporaryFile("w+", suffix=".csv", delete=False)
+    REASONS = {0x8: "hw_slowdown", 0x40: "hw_thermal_slowdown", 0x20: "sw_thermal_slowdown", 0x4: "sw_power_cap"}
+
+    def __init__(self, torch_device_index):
+        self.samples = []
+        self.stop_flag = False
+        self.h = None
+        self.idx = torch_device_index
         try:
-            self.proc = subprocess.Popen(["nvidia-smi", "-i", str(index), f"--query-gpu={self.FIELDS}",
-                                          "--format=csv,noheader,nounits", "-lms", "100"], stdout=self.tmp, stderr=subprocess.DEVNULL)
+            import pynvml
+            import torch
+            pynvml.nvmlInit()
+            self.nv = pynvml
+            try:
+                uuid = str(torch.cuda.get_device_properties(torch_device_index).uuid)
+                self.h = pynvml.nvmlDeviceGetHandleByUUID(("GPU-" + uuid).encode() if not uuid.startswith("GPU-") else uuid.encode())
+            except Exception:
+                self.h = pynvml.nvmlDeviceGetHandleByIndex(torch_device_index)
+            self.max_sm = float(pynvml.nvmlDeviceGetMaxClockInfo(self.h, pynvml.NVML_CLOCK_SM))
         except Exception:
-            self.proc = None
+            self.h = None
+        self.thread = threading.Thread(target=self._run, daemon=True)
+
+    def _one(self):
+        nv = self.nv
+        sm = float(nv.nvmlDeviceGetClockInfo(self.h, nv.NVML_CLOCK_SM))
+        try:
+            reasons = int(nv.nvmlDeviceGetCurrentClocksEventReasons(self.h))
+        except Exception:
+            reasons = int(nv.nvmlDeviceGetCurrentClocksThrottleReasons(self.h))
+        try:
+            pw = nv.nvmlDeviceGetPowerUsage(self.h) / 1000.0
+        except Exception:
+            pw = None
+        return sm, reasons, pw
+
+    def _run(self):
+        while not self.stop_flag:
+            try:
+                self.samples.append(self._one())
+            except Exception:
+                break
+            time.sleep(0.002)
+
+    def start(self):
+        if self.h is not None:
+            self.thread.start()
+        return self
 
     def stop(self):
-        out = {"sm_mhz": None, "sm_max_mhz": None, "reasons": []}
-        if self.proc is None:
-            return out
-        self.proc.terminate()
+        out = {"sm_mhz": None, "sm_max_mhz": None, "reasons": [], "how": "NVML polled every ~2 ms by a host thread during the timed batches"}
+        if self.h is None:
+            return self._smi(out)
         try:
-            self.proc.wait(timeout=5)
+            self.samples.append(self._one())          # the queue of the last batch is still draining here
         except Exception:
-            self.proc.kill()
-        self.tmp.flush()
-        rows = [r.split(",") for r in open(self.tmp.name).read().strip().splitlines() if r.count(",") >= 6]
-        os.unlink(self.tmp.name)
-        if not rows:
-            return out
+            pass
+        self.stop_flag = True
+        self.thread.join(timeout=2)
+        if not self.samples:
+            return self._smi(out)
+        sm = sorted(s[0] for s in self.samples)
+        bits = 0
+        for s in self.samples:
+            bits |= s[1]
+        out.update(sm_mhz=sm[len(sm) // 2], sm_min_mhz=sm[0], sm_max_mhz=self.max_sm, samples=len(sm),
+                   reasons=[nm for b, nm in self.REASONS.items() if bits & b])
+        pws = [s[2] for s in self.samples if s[2] is not None]
+        if pws:
+            out["power_w_max"] = max(pws)
+        return out
+
+    def _smi(self, out):
         try:
-            sm = sorted(float(r[0]) for r in rows)
-            out["sm_mhz"] = sm[len(sm) // 2]
-            out["sm_max_mhz"] = float(rows[0][1])
-            out["power_w_max"] = max(float(r[2]) for r in rows)
+            q = "clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown," \
+                "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap"
+            r = subprocess.run(["nvidia-smi", "-i", str(self.idx), f"--query-gpu={q}", "--format=csv,noheader,nounits"],
+                               capture_output=True, text=True, timeout=10).stdout.strip().split(",")
             names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
-            out["reasons"] = [nm for i, nm in enumerate(names) if any(r[3 + i].strip() == "Active" for r in rows)]
-            out["samples"] = len(rows)
+            out.update(sm_mhz=float(r[0]), sm_max_mhz=float(r[1]), power_w_max=float(r[2]),
+                       reasons=[nm for i, nm in enumerate(names) if r[3 + i].strip() == "Active"],
+                       how="one nvidia-smi query right after the timed batches (NVML unavailable)")
         except Exception:
             pass
         return out
 
 
+def oracle_timing(wl, budget_s, threads=None):
+    """The oracle as it stands (oracle/pfo.c) on the host cores: full FS steps of the workload until budget_s is spent."""
+    import ctypes
+    from oracle import pfo
+    pfo.build()
+    n, p, prec, init, dt, _ = WORKLOADS[wl]
+    c, eta, dx = make_fields(wl)
+    m = pfo.Model(n=n, n_eta=p, dx=dx, dt=dt)
+    gomp, before = None, pfo.num_threads()
+    if threads is not None:
+        try:                                          # the oracle's OpenMP runtime; nothing in oracle/ is changed
+            gomp = ctypes.CDLL("libgomp.so.1")
+            gomp.omp_set_num_threads(int(threads))
+        except Exception:
+            return None
+    used = pfo.num_threads()
+    t0 = time.time()
+    k = 0
+    while k < 2 or (time.time() - t0 < budget_s and k < 200):
+        c, eta = m.step_fs(c, eta, 1)
+        k += 1
+        if time.time() - t0 > 3 * budget_s:
+            break
+    el = time.time() - t0
+    if gomp is not None:
+        gomp.omp_set_num_threads(int(before))
+    return {"value": k / el, "unit": "steps/s", "cores": used, "kind": "oracle",
+            "sample": f"{k} full FS steps of the same workload ({el:.1f} s)"}
+
+
 def run_reference(args):
-    """The oracle (oracle/pfo.c, as it stands) on the host cores: the base contract's reference arm for this tier."""
-    rank = int(os.environ.get("RANK", "0"))
-    if rank != 0:
+    """The oracle (oracle/pfo.c, as it stands) on the host cores: the base contract's reference arm for this tier.
+    Under torchrun rank 0 alone runs and prints; the other ranks exit 0 without work."""
+    if int(os.environ.get("RANK", "0")) != 0:
         return
     from oracle import pfo
     pfo.build()
@@ -145,7 +248,8 @@ def run_reference(args):
     m = pfo.Model(n=n, n_eta=p, dx=dx, dt=dt)
     budget = float(os.environ.get("PF_REF_BUDGET_S", "150"))
     t_all = time.time()
-    for _ in range(min(args.warmup, 1)):
+    W = min(args.warmup, 1)
+    for _ in range(W):
         c, eta = m.step_fs(c, eta, 1)
     t0 = time.time()
     done = 0
@@ -156,14 +260,19 @@ def run_reference(args):
     val = done / el
     N = int(np.prod(n))
     line = {"impl": "reference", "metric": METRIC, "value": val, "unit": "steps/s", "n_gpus": args.gpus, "steps": done,
-            "warmup": min(args.warmup, 1), "ms_per_step": 1e3 * el / done, "higher_is_better": True, "scaling": "weak",
+            "warmup": W, "ms_per_step": 1e3 * el / done, "higher_is_better": True, "scaling": "weak",
             "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-            "config": {"workload": desc, "init": init, "dt": dt, "note": "CPU oracle; steps bounded by a time budget"},
+            "config": {"workload": desc, "init": init_name(init), "dt": dt,
+                       "note": "CPU oracle (oracle/pfo.c as it stands); steps bounded by a time budget"},
             "gpoint_updates_per_s": val * N / 1e9,
             "cpu_baseline": {"value": val, "unit": "steps/s", "cores": pfo.num_threads(), "kind": "oracle",
                              "sample": f"{done} full FS steps of the same workload"},
             "e2e": {"value": val, "unit": "steps/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}}
     print(json.dumps(line), flush=True)
+
+
+def init_name(init):
+    return "Eqs. 4-6 benchmark field (synth.init_b)" if init == "B" else "seeded noise (synth.init_a)"
 
 
 def cufft_side_reference(torch, n, p, prec, dx, dt, c0, eta0, stream, steps=20):
@@ -216,33 +325,31 @@ def cufft_side_reference(torch, n, p, prec, dx, dt, c0, eta0, stream, steps=20):
             "what": "torch.fft.rfftn/irfftn (cuFFT) + elementwise torch ops, single simulation, same workload"}
 
 
-def run_ours(args):
-    import torch
-    import torch.distributed as dist
-    from paper_2306_04322_b200 import pf, replicas
+def stats(vals):
+    v = sorted(vals)
+    return {"min": v[0], "median": v[len(v) // 2] if len(v) % 2 else 0.5 * (v[len(v) // 2 - 1] + v[len(v) // 2]), "max": v[-1], "n": len(v)}
 
-    rank = int(os.environ.get("RANK", "0"))
-    world = int(os.environ.get("WORLD_SIZE", "1"))
-    local = int(os.environ.get("LOCAL_RANK", "0"))
-    if not torch.cuda.is_available():
-        raise SystemExit("bench.py needs a CUDA device (there is no CPU fallback)")
-    torch.cuda.set_device(local)
-    if world > 1:
-        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
-    pf.lib()                                   # fails loudly if libpf.so is missing
 
-    n, p, prec, init, dt, desc = WORKLOADS[args.workload]
+def measure_workload(wl, K, W, env, full=True):
+    """All device measurements of one workload. Returns the dict of a JSON line (headline keys + details).
+    env: torch, dist, pf, replicas, rank, world, stream."""
+    torch, dist, pf, replicas = env["torch"], env["dist"], env["pf"], env["replicas"]
+    rank, world, stream = env["rank"], env["world"], env["stream"]
+    n, p, prec, init, dt, desc = WORKLOADS[wl]
     w = 8 if prec == "f64" else 4
     F, N = p + 1, int(np.prod(n))
     R = N * w
-    c0, eta0, dx = make_fields(args.workload)
+    c0, eta0, dx = make_fields(wl)
     # replicas only (DESIGN.md "Multi-GPU"): every rank advances its own independent simulations
     state_bytes = (F + 1) * R if len(n) == 2 else 3 * F * R
     reps = 1 if state_bytes > 2 * L2_BYTES else int(np.ceil(2.5 * L2_BYTES / state_bytes))
-    stream = torch.cuda.Stream()
     ctxs = [pf.Context(n, n_eta=p, dx=dx, dt=dt, precision=prec, stream=stream.cuda_stream) for _ in range(reps)]
-    for i, cx in enumerate(ctxs):
-        cx.set_fields(replicas.perturb(c0, rank, i, reps), eta0)
+
+    def reset_fields(group, count):
+        for i, cx in enumerate(group):
+            cx.set_fields(replicas.perturb(c0, rank, i, count), eta0)
+
+    reset_fields(ctxs, reps)
     torch.cuda.synchronize()
 
     def barrier():
@@ -250,154 +357,151 @@ def run_ours(args):
             dist.barrier()
         torch.cuda.synchronize()
 
-    def run_steps(k, which):
-        # one step of each replica in turn; a call is asynchronous (graph replay of one step)
-        for s in range(k):
-            which[s % len(which)].step_fs(1)
-
-    def timed(k, which):
+    def timed(fn):
         e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
         barrier()
         e0.record(stream)
-        run_steps(k, which)
+        fn()
         e1.record(stream)
         barrier()
         return replicas.max_over_ranks(e0.elapsed_time(e1), device="cuda")
 
-    K, W = args.steps, max(args.warmup, 3)
-    run_steps(W * len(ctxs), ctxs)
-    sampler = ClockSampler(torch.cuda.current_device()) if rank == 0 else None
+    def fs_steps(k, which):
+        for s in range(k):                     # one step of each replica in turn; a call is asynchronous (graph replay)
+            which[s % len(which)].step_fs(1)
+
+    nbatch = max(5, min(50, int(np.ceil(1000 / K))))
+    fs_steps(max(W, 3) * len(ctxs), ctxs)
+    sampler = ClockSampler(torch.cuda.current_device()).start() if rank == 0 else None
     l0 = sum(cx.launch_count() for cx in ctxs)
-    ms = timed(K, ctxs)
-    launches = sum(cx.launch_count() for cx in ctxs) - l0
+    batches = [timed(lambda: fs_steps(K, ctxs)) for _ in range(nbatch)]
+    launches = (sum(cx.launch_count() for cx in ctxs) - l0) // nbatch
     clocks = sampler.stop() if sampler else {}
+    bst = stats(batches)
+    ms = bst["median"]
     value = replicas.job_throughput(K, ms, world)
+    step_ms = ms / K
 
     # single simulation, state resident in L2 where it fits (reported, not the headline)
-    ms_res = timed(K, ctxs[:1])
-    resident = replicas.job_throughput(K, ms_res, world)
+    res_b = [timed(lambda: fs_steps(K, ctxs[:1])) for _ in range(5)]
+    resident = replicas.job_throughput(K, stats(res_b)["median"], world)
 
-    # per-kernel device times: CUDA events on the context's stream, recorded by the library around PROF_REPEAT back-to-back
-    # launches of each kernel (pf_set_profiling), same replica cycling as the timed region. Timing only: the replicas'
-    # fields are not a trajectory afterwards (the e2e leg below sets fields again).
-    for cx in ctxs:
-        cx.set_profiling(PROF_REPEAT)
-    acc, cnt = {}, 0
-    for s in range(min(K, 20 * len(ctxs))):
-        cx = ctxs[s % len(ctxs)]
-        cx.step_fs(1)
-        for name, t in cx.fs_kernel_times():
-            acc[name] = acc.get(name, 0.0) + t
-        cnt += 1
-    for cx in ctxs:
-        cx.set_profiling(0)
-    kms = {k: v / cnt for k, v in acc.items()}
+    # per-kernel device times, L2-cold like the step: kernel k of every replica in turn (pf_launch_fs_kernel) between two
+    # events on the stream, repeated; the replicas' fields are no trajectory afterwards (they are set again below)
+    names = ctxs[0].fs_kernel_names()
+    kms = {}
+    rounds = max(2, int(np.ceil(40 / len(ctxs))))
+    for k, name in enumerate(names):
+        def one_kernel():
+            for _ in range(rounds):
+                for cx in ctxs:
+                    cx.launch_fs_kernel(k)
+        one_kernel()
+        ts = [timed(one_kernel) for _ in range(5)]
+        kms[name] = stats(ts)["median"] / (rounds * len(ctxs))
+    reset_fields(ctxs, reps)
     ksurvey, kdesign = bytes_model(n, p, w)
     survey_bytes, design_bytes = sum(ksurvey.values()), sum(kdesign.values())
     peak, peak_src = peaks()
     dom = max(kms, key=kms.get)
     achieved = ksurvey[dom] / (kms[dom] * 1e-3) / 1e9
+    traffic, traffic_src = ncu_traffic(wl, dom)
     roofline = {"bound": "hbm", "kernel": dom, "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
-                "traffic": NCU_TRAFFIC.get(args.workload, {}).get(dom), "peak_source": peak_src,
+                "traffic": traffic, "traffic_source": traffic_src, "peak_source": peak_src,
                 "algorithmic_bytes_per_launch": ksurvey[dom],
                 "algorithmic_bytes_note": "SURVEY 8(d) per-pass bytes of the passes this kernel fuses (see DESIGN.md section 5)",
                 "design_bytes_per_launch": kdesign[dom],
                 "achieved_vs_design_bytes": kdesign[dom] / (kms[dom] * 1e-3) / 1e9,
-                "kernel_ms": kms[dom], "kernels_ms": kms, "kernel_timing": f"events around {PROF_REPEAT} back-to-back launches of one kernel on one replica (L2 warm after the first; the step time above is the cold-L2 figure)",
+                "frac_vs_design_bytes": kdesign[dom] / (kms[dom] * 1e-3) / 1e9 / peak,
+                "kernel_ms": kms[dom], "kernels_ms": kms,
+                "kernel_timing": f"CUDA events on the launch stream around {rounds * len(ctxs)} launches of this kernel alone, "
+                                 f"one per replica in turn ({len(ctxs)} replicas: L2-cold like the step), plain launches",
                 "kernel_share_of_step": kms[dom] / sum(kms.values())}
-    step_ms = ms / K
     step_roofline = {"bytes_per_step_survey_8d": survey_bytes, "bytes_per_step_this_design": design_bytes,
                      "achieved_vs_survey_bytes_gbs": survey_bytes / (step_ms * 1e-3) / 1e9,
                      "frac_vs_survey_bytes": survey_bytes / (step_ms * 1e-3) / 1e9 / peak,
                      "achieved_vs_design_bytes_gbs": design_bytes / (step_ms * 1e-3) / 1e9,
                      "frac_vs_design_bytes": design_bytes / (step_ms * 1e-3) / 1e9 / peak}
 
-    # end to end through the C ABI with HOST buffers: set (H2D) + 1 step + get (D2H), pinned host memory
+    line = {"metric": METRIC, "value": value, "unit": "steps/s", "n_gpus": world, "steps": K, "warmup": max(W, 3),
+            "ms_per_step": step_ms, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": prec,
+            "data": "synthetic",
+            "config": {"workload": desc, "init": init_name(init), "dt": dt, "replicas_per_gpu": reps,
+                       "parallelism": "independent replicas per GPU, no collective",
+                       "l2": (f"timed loop cycles {reps} independent replicas ({reps * state_bytes / 1e6:.0f} MB of state > 126 MB L2)"
+                              if reps > 1 else f"state {state_bytes / 1e6:.0f} MB per step exceeds the 126 MB L2")},
+            "timed_batches": {"steps_per_batch": K, "batches": nbatch, "ms": bst,
+                              "steps_per_s": {"min": replicas.job_throughput(K, bst["max"], world),
+                                              "median": value, "max": replicas.job_throughput(K, bst["min"], world)},
+                              "note": "value = the median batch; every batch is K steps bracketed by barrier + synchronize, CUDA events on the launch stream, max over ranks"},
+            "gpoint_updates_per_s": value * N / 1e9,
+            "field_point_updates_per_s_G": value * N * F / 1e9,
+            "l2_resident_single_simulation": {"value": resident, "unit": "steps/s", "gpoint_updates_per_s": resident * N / 1e9},
+            "roofline": roofline, "step_roofline": step_roofline, "gpu_launches": int(launches), "clocks": clocks}
+
+    # end to end through the C ABI with HOST buffers: set (H2D) + 1 step + get (D2H), pinned host memory, ONE simulation
     tdt = torch.float64 if prec == "f64" else torch.float32
-    hc = torch.empty(tuple(reversed(n)), dtype=tdt).pin_memory()
-    he = torch.empty((p,) + tuple(reversed(n)), dtype=tdt).pin_memory()
-    hc.numpy()[...] = c0
-    he.numpy()[...] = eta0
     L = pf.lib()
-    cx = ctxs[0]
-    ke = max(3, min(K, 20))
-    def e2e_step():
-        L.pf_set_fields(cx._h, hc.data_ptr(), he.data_ptr(), pf.PF_HOST)
-        L.pf_step_fs(cx._h, 1)
-        L.pf_get_fields(cx._h, hc.data_ptr(), he.data_ptr(), pf.PF_HOST)
-    for _ in range(2):
-        e2e_step()
-    barrier()
-    t0 = time.perf_counter()
-    for _ in range(ke):
-        e2e_step()
-    torch.cuda.synchronize()
-    e2e_s = time.perf_counter() - t0
-    e2e_s = replicas.max_over_ranks(e2e_s, device="cuda")
-    serial_e2e = world * ke / e2e_s
-    # the same loop for two independent simulations from two host threads (own context, stream and pinned buffers
-    # each): the H2D copy of one overlaps the D2H copy of the other (PCIe is full duplex)
-    import threading
-    cxs2 = [pf.Context(n, n_eta=p, dx=dx, dt=dt, precision=prec) for _ in range(2)]
-    bufs2 = []
-    for _ in range(2):
+
+    def host_buffers():
         bc = torch.empty(tuple(reversed(n)), dtype=tdt).pin_memory()
         be = torch.empty((p,) + tuple(reversed(n)), dtype=tdt).pin_memory()
         bc.numpy()[...] = c0
         be.numpy()[...] = eta0
-        bufs2.append((bc, be))
+        return bc, be
 
-    def worker(i, steps):
-        h, (bc, be) = cxs2[i]._h, bufs2[i]
+    def e2e_loop(h, bufs, steps):
+        bc, be = bufs
         for _ in range(steps):
             L.pf_set_fields(h, bc.data_ptr(), be.data_ptr(), pf.PF_HOST)
             L.pf_step_fs(h, 1)
             L.pf_get_fields(h, bc.data_ptr(), be.data_ptr(), pf.PF_HOST)
 
-    for i in range(2):
-        worker(i, 2)
+    ke = max(3, min(K, 20))
+    bufs = host_buffers()
+    e2e_loop(ctxs[0]._h, bufs, 2)
     barrier()
     t0 = time.perf_counter()
-    th = [threading.Thread(target=worker, args=(i, ke)) for i in range(2)]
-    for t in th:
-        t.start()
-    for t in th:
-        t.join()
+    e2e_loop(ctxs[0]._h, bufs, ke)
     torch.cuda.synchronize()
-    e2e2_s = replicas.max_over_ranks(time.perf_counter() - t0, device="cuda")
-    for cx2 in cxs2:
-        cx2.close()
-    e2e = {"value": world * 2 * ke / e2e2_s, "unit": "steps/s", "h2d_bytes_per_step": F * R, "d2h_bytes_per_step": F * R,
-           "steps": 2 * ke, "contexts": 2, "one_context_value": serial_e2e,
-           "note": "pf_set_fields(HOST) + pf_step_fs(1) + pf_get_fields(HOST) per step, pinned host buffers; two independent "
-                   "simulations driven from two host threads so that uploads and downloads overlap; one_context_value = the same loop for one simulation"}
-
-    line = {"metric": METRIC, "value": value, "unit": "steps/s", "n_gpus": world, "steps": K, "warmup": W,
-            "ms_per_step": step_ms, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": prec,
-            "data": "synthetic",
-            "config": {"workload": desc, "init": "Eqs. 4-6 benchmark field (synth.init_b)" if init == "B" else "seeded noise (synth.init_a)",
-                       "dt": dt, "replicas_per_gpu": reps, "parallelism": "independent replicas per GPU, no collective",
-                       "l2": (f"timed loop cycles {reps} independent replicas ({reps * state_bytes / 1e6:.0f} MB of state > 126 MB L2)"
-                              if reps > 1 else f"state {state_bytes / 1e6:.0f} MB per step exceeds the 126 MB L2")},
-            "gpoint_updates_per_s": value * N / 1e9,
-            "field_point_updates_per_s_G": value * N * F / 1e9,
-            "l2_resident_single_simulation": {"value": resident, "unit": "steps/s", "gpoint_updates_per_s": resident * N / 1e9},
-            "roofline": roofline, "step_roofline": step_roofline, "e2e": e2e, "gpu_launches": int(launches), "clocks": clocks}
+    e2e_s = replicas.max_over_ranks(time.perf_counter() - t0, device="cuda")
+    e2e = {"value": world * ke / e2e_s, "unit": "steps/s", "h2d_bytes_per_step": F * R, "d2h_bytes_per_step": F * R,
+           "steps": ke, "contexts": 1,
+           "note": "pf_set_fields(HOST) + pf_step_fs(1) + pf_get_fields(HOST) per step of ONE simulation, pinned host buffers, "
+                   "host wall clock around the loop (PCIe bound)"}
+    if full:
+        # two independent simulations from two host threads (own context, stream and pinned buffers each): the upload of
+        # one overlaps the download of the other (PCIe is full duplex). Reported beside the single-simulation value.
+        cxs2 = [pf.Context(n, n_eta=p, dx=dx, dt=dt, precision=prec) for _ in range(2)]
+        bufs2 = [host_buffers() for _ in range(2)]
+        for i in range(2):
+            e2e_loop(cxs2[i]._h, bufs2[i], 2)
+        barrier()
+        t0 = time.perf_counter()
+        th = [threading.Thread(target=e2e_loop, args=(cxs2[i]._h, bufs2[i], ke)) for i in range(2)]
+        for t in th:
+            t.start()
+        for t in th:
+            t.join()
+        torch.cuda.synchronize()
+        e2e2_s = replicas.max_over_ranks(time.perf_counter() - t0, device="cuda")
+        for cx2 in cxs2:
+            cx2.close()
+        e2e["two_contexts_value"] = world * 2 * ke / e2e2_s
+    line["e2e"] = e2e
 
     # independent simulations advanced concurrently on two streams (the paper's sweeps are independent runs, DESIGN.md
     # "Multi-GPU"): kernels of different simulations fill each other's tails. Reported beside the headline, which stays
     # the one-stream figure. Timed with events on `stream`, which waits for the second stream's last step.
-    concurrent = None
-    if len(ctxs) >= 2:
+    if full and len(ctxs) >= 2:
         stream2 = torch.cuda.Stream()
         half = max(1, len(ctxs) // 2)
         ctxs2 = [pf.Context(n, n_eta=p, dx=dx, dt=dt, precision=prec, stream=stream2.cuda_stream) for _ in range(half)]
-        for i, cx in enumerate(ctxs2):
-            cx.set_fields(replicas.perturb(c0, rank, i, half), eta0)
+        reset_fields(ctxs2, half)
+        for cx in ctxs2:
             cx.step_fs(W)
         grpa = ctxs[:half]
-        for i, cx in enumerate(grpa):          # the profiling leg left these replicas without a valid trajectory
-            cx.set_fields(replicas.perturb(c0, rank, i, reps), eta0)
+        for cx in grpa:
             cx.step_fs(W)
         barrier()
         c0e, c1e, c2e = (torch.cuda.Event(enable_timing=True) for _ in range(3))
@@ -411,53 +515,89 @@ def run_ours(args):
         c1e.record(stream)
         barrier()
         cms = replicas.max_over_ranks(c0e.elapsed_time(c1e), device="cuda")
-        concurrent = {"streams": 2, "value": replicas.job_throughput(2 * (K // 2), cms, world), "unit": "steps/s",
-                      "us_per_step": 1e3 * cms / (2 * (K // 2)),
-                      "note": "two independent simulations in flight at a time, one per stream; every simulation still advances step by step"}
+        line["concurrent_replicas"] = {"streams": 2, "value": replicas.job_throughput(2 * (K // 2), cms, world), "unit": "steps/s",
+                                       "us_per_step": 1e3 * cms / (2 * (K // 2)),
+                                       "note": "two independent simulations in flight at a time, one per stream; every simulation still advances step by step"}
         for cx in ctxs2:
             cx.close()
 
-    # comparison path: explicit FD steps of one simulation of the same grid, device-timed
-    fd = pf.Context(n, n_eta=p, dx=dx, dt=1e-6, precision=prec, stream=stream.cuda_stream)
-    fd.set_fields(c0, eta0)
-    kfd = max(20, min(2000, K // 4))
-    fd.step_fd(20)
-    f0, f1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    barrier()
-    f0.record(stream)
-    fd.step_fd(kfd)
-    f1.record(stream)
-    barrier()
-    fd_ms = f0.elapsed_time(f1) / kfd
-    fd.close()
+    # comparison path: explicit FD steps, same replica cycling as the FS loop (L2-cold against L2-cold)
+    for cx in ctxs:
+        cx.set_dt(1e-6)
+    reset_fields(ctxs, reps)
+
+    def fd_steps(k, which):
+        for s in range(k):
+            which[s % len(which)].step_fd(1)
+
+    kfd = max(20 * len(ctxs), min(2000, K))
+    fd_steps(3 * len(ctxs), ctxs)
+    fd_ms = stats([timed(lambda: fd_steps(kfd, ctxs)) for _ in range(5)])["median"] / kfd
+    fd_res_ms = stats([timed(lambda: fd_steps(kfd, ctxs[:1])) for _ in range(3)])["median"] / kfd
     fd_bytes = 2 * F * R                      # fused kernels: every field read once and written once per step
-    if concurrent:
-        line["concurrent_replicas"] = concurrent
     line["fd_comparison_path"] = {"value": 1e3 / fd_ms, "unit": "steps/s", "us_per_step": 1e3 * fd_ms, "steps": kfd,
                                   "algorithmic_bytes_per_step": fd_bytes, "achieved_gbs": fd_bytes / (fd_ms * 1e-3) / 1e9,
-                                  "note": "explicit forward-Euler 5/7-point step (pf_step_fd), single simulation (L2 resident below ~60 MB of state)",
+                                  "frac_of_hbm_peak": fd_bytes / (fd_ms * 1e-3) / 1e9 / peak,
+                                  "l2_resident_single_simulation_us_per_step": 1e3 * fd_res_ms,
+                                  "note": f"explicit forward-Euler 5/7-point step (pf_step_fd), one launch per step, cycling the same {len(ctxs)} replicas as the FS loop",
                                   "fs_over_fd_time_per_step": step_ms / fd_ms}
+    for cx in ctxs:
+        cx.set_dt(dt)
 
-    if rank == 0 and not args.no_cufft:
+    if rank == 0 and full and not env["args"].no_cufft:
         line["cufft_side_reference"] = cufft_side_reference(torch, n, p, prec, dx, dt, c0, eta0, stream)
-
-    if rank == 0 and world == 1 and not args.no_cpu_baseline:
-        from oracle import pfo
-        pfo.build()
-        m = pfo.Model(n=n, n_eta=p, dx=dx, dt=dt)
-        cc, ee = c0, eta0
-        t0 = time.time()
-        k = 0
-        while k < 3 or (time.time() - t0 < 10 and k < 50):
-            cc, ee = m.step_fs(cc, ee, 1)
-            k += 1
-            if time.time() - t0 > 40:
-                break
-        el = time.time() - t0
-        line["cpu_baseline"] = {"value": k / el, "unit": "steps/s", "cores": pfo.num_threads(), "kind": "oracle",
-                                "sample": f"{k} full FS steps of the same workload ({el:.1f} s)"}
     for cx in ctxs:
         cx.close()
+    return line
+
+
+def spawn_ranks(args, argv):
+    """python bench.py --gpus N outside torchrun: re-execute under torch.distributed.run with N ranks on this node."""
+    port = 29500 + (os.getpid() % 2000)
+    cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", f"--nproc-per-node={args.gpus}",
+           "--master-addr", "127.0.0.1", "--master-port", str(port), os.path.abspath(__file__)] + argv
+    return subprocess.call(cmd)
+
+
+def run_ours(args):
+    import torch
+    import torch.distributed as dist
+    from paper_2306_04322_b200 import pf, replicas
+
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if os.environ.get("PF_LIBPF") and not args.allow_lib_override:
+        raise SystemExit("PF_LIBPF is set: bench.py times the product library only (ablation builds: --allow-lib-override)")
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device (there is no CPU fallback)")
+    torch.cuda.set_device(local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    pf.lib()                                   # fails loudly if libpf.so is missing
+    env = {"torch": torch, "dist": dist, "pf": pf, "replicas": replicas, "rank": rank, "world": world,
+           "stream": torch.cuda.Stream(), "args": args}
+
+    K = args.steps if args.steps is not None else DEFAULT_STEPS[args.workload]
+    line = measure_workload(args.workload, K, args.warmup, env, full=True)
+    line["library"] = {"path": pf.SO_PATH, "override": bool(os.environ.get("PF_LIBPF")), "kernel_source_hash": kernel_source_hash()}
+
+    if rank == 0 and world == 1 and not args.no_cpu_baseline:
+        allc = oracle_timing(args.workload, 8.0)
+        one = oracle_timing(args.workload, 4.0, threads=1)
+        line["cpu_baseline"] = dict(allc, single_thread=one)
+
+    others = {}
+    for wl in args.also:
+        if wl == args.workload:
+            continue
+        Ko = min(K, DEFAULT_STEPS[wl]) if args.steps is not None else DEFAULT_STEPS[wl]
+        sub = measure_workload(wl, Ko, args.warmup, env, full=False)
+        if rank == 0 and world == 1 and not args.no_cpu_baseline:
+            sub["cpu_baseline"] = oracle_timing(wl, 5.0)
+        others[wl] = sub
+    if others:
+        line["workloads"] = others
     if rank == 0:
         print(json.dumps(line), flush=True)
     if world > 1:
@@ -467,16 +607,24 @@ def run_ours(args):
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=None, help="default: enough steps for a >= 1 s timed region")
+    ap.add_argument("--steps", type=int, default=None, help="steps per timed batch (default: >= 200, per workload)")
     ap.add_argument("--warmup", type=int, default=5)
     ap.add_argument("--workload", default="1024sq", choices=sorted(WORKLOADS))
+    ap.add_argument("--also", nargs="*", default=None, choices=sorted(WORKLOADS),
+                    help="further workloads measured in the same invocation and reported under 'workloads' "
+                         "(default: 256cube beside the default headline, none otherwise)")
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-cufft", action="store_true", help="skip the cuFFT side reference")
+    ap.add_argument("--allow-lib-override", action="store_true", help="accept PF_LIBPF (ablation builds; never for a reported number)")
     args = ap.parse_args()
-    if args.steps is None:
-        args.steps = DEFAULT_STEPS[args.workload] if args.impl == "ours" else 20
+    if args.also is None:
+        args.also = ["256cube"] if args.workload == "1024sq" else []
+    if args.gpus > 1 and "RANK" not in os.environ:
+        raise SystemExit(spawn_ranks(args, sys.argv[1:]))
     if args.impl == "reference":
+        if args.steps is None:
+            args.steps = 20
         run_reference(args)
     else:
         run_ours(args)

@@ -24,6 +24,8 @@
  *   - all work is queued on pf_params.stream (a cudaStream_t passed as void*; borrowed, never destroyed;
  *     NULL = a private blocking stream of the context, which orders with the legacy default stream). pf_step_* and device-side set/get are asynchronous;
  *     pf_get_fields(PF_HOST), pf_set_fields(PF_HOST) and pf_free_energy synchronise that stream;
+ *   - a context belongs to the CUDA device that was current in pf_create; every later call must be made with that
+ *     device current (PF_EINVAL otherwise);
  *   - every call returns PF_OK (0) or a negative code; nothing throws or aborts. After PF_ECUDA
  *     pf_last_cuda_error gives the CUDA error string.
  */
@@ -59,7 +61,8 @@ typedef struct {
 /* Creates a context on the CURRENT CUDA device: validates p, allocates all device buffers, builds
  * the twiddle and frequency tables. *out is set only on PF_OK.
  * PF_EINVAL: null pointers, ndim not 2/3, dt <= 0, dx <= 0, n_eta out of range, bad enum values;
- * PF_EUNSUPPORTED: a grid size that is not a power of two in 16..2048 (nz must be 1 in 2D);
+ * PF_EUNSUPPORTED: a grid size that is not a power of two in 16..2048 (nz must be 1 in 2D); every combination of
+ *   grid size, n_eta 0..8 and precision that passes this check can be stepped (tests sweep them);
  * PF_ENOMEM: device allocation failed; PF_ECUDA: no usable device / a CUDA call failed. */
 int pf_create(const pf_params *p, pf_ctx **out);
 
@@ -101,15 +104,20 @@ long long pf_launch_count(const pf_ctx *ctx);
 /* Device time in milliseconds spent by kernel `which` of the most recent pf_step_fs call, measured
  * with CUDA events on the context's stream when profiling was switched on with pf_set_profiling
  * (which = 0 .. pf_num_fs_kernels()-1, in launch order within one step; averaged over the steps of
- * that call). Returns a negative value when unavailable. Profiling disables CUDA-graph replay.
- * pf_set_profiling(ctx, R): R = 0 switches it off; R = 1 brackets every kernel of a step with events; R > 1 launches
- * every kernel R times back to back between its two events and reports elapsed / R, which removes the event and
- * launch overhead from the per-kernel figure -- the fields are then NOT a valid trajectory (each kernel was applied
- * R times): call pf_set_fields before stepping again. */
+ * that call). Returns a negative value when unavailable. Profiling (on != 0) disables CUDA-graph replay and
+ * programmatic dependent launch; the trajectory is the same. A single bracketed launch carries a few microseconds
+ * of event overhead: for per-kernel figures without it use pf_launch_fs_kernel. */
 int    pf_set_profiling(pf_ctx *ctx, int on);
 int    pf_num_fs_kernels(const pf_ctx *ctx);
 double pf_fs_kernel_ms(pf_ctx *ctx, int which);
 const char *pf_fs_kernel_name(const pf_ctx *ctx, int which);
+
+/* Timing aid: queues ONLY kernel `which` (0 .. pf_num_fs_kernels()-1) of one Fourier-spectral step on the context's
+ * stream (asynchronous, plain launch). A caller brackets a sequence of such calls -- e.g. the same kernel of several
+ * contexts whose combined state exceeds the L2 -- with its own events. Needs fields (PF_ESTATE otherwise). Afterwards
+ * the buffers are no trajectory: pf_step_*, pf_get_fields and pf_free_energy return PF_ESTATE until the next
+ * pf_set_fields, further pf_launch_fs_kernel calls are allowed. */
+int    pf_launch_fs_kernel(pf_ctx *ctx, int which);
 
 const char *pf_strerror(int code);
 const char *pf_last_cuda_error(const pf_ctx *ctx);      /* "" when none */

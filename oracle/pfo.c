@@ -424,3 +424,19 @@ int pfo_free_energy(const pfo_params *p, const double *c, const double *eta, int
     out[0] = total;
     return 0;
 }
+
+/* ------------------------------------------------------------------------------------------
+ * Eq. 22: E_phi = int (phi_0 - phi)^2 dV / int phi_0^2 dV on a uniform grid.
+ * ---------------------------------------------------------------------------------------- */
+double pfo_error_eq22(long n, const double *phi, const double *ref)
+{
+    if (n <= 0 || !phi || !ref) return -1.0;
+    double num = 0.0, den = 0.0;
+    for (long i = 0; i < n; ++i) {
+        double d = ref[i] - phi[i];
+        num += d * d;
+        den += ref[i] * ref[i];
+    }
+    if (!(den > 0.0)) return -1.0;
+    return num / den;
+}

@@ -16,8 +16,9 @@
  * Pins (tests/test_oracle_*.py, all "-m 'not gpu'"): brute-force DFT vs radix-2 vs numpy.fft;
  * central differences of f_chem; closed-form amplification factors of single Fourier modes
  * (FS and FD); conservation of mean c; monotone free energy; 5/7-point Laplacian == F^-1[-|xi_c2|^2 F u];
- * spectral Laplacian exact on band-limited fields; closed-form free-energy integrals; the
- * paper's printed FD time steps against the linear stability bound.
+ * spectral Laplacian exact on band-limited fields; closed-form free-energy integrals (2D and 3D,
+ * both gradient kinds); Eq. 22 on cosines of known amplitude; the paper's printed FD time steps
+ * against the linear stability bound.
  * Parity unpinned: full trajectories against the paper's figures (Figs. 1-6 are images and the
  * paper's pre-evolved initial fields are not available) -- see DESIGN.md.
  *
@@ -77,6 +78,12 @@ int    pfo_step_fd(const pfo_params *p, double *c, double *eta, int nsteps);
  * out[0] total, out[1] chemical, out[2] kappa_c/2 |grad c|^2, out[3+i] kappa_eta/2 |grad eta_i|^2.
  * gradient_kind 0: Parseval with the k2_kind frequencies; 1: forward differences. */
 int    pfo_free_energy(const pfo_params *p, const double *c, const double *eta, int gradient_kind, double *out);
+
+/* L2 normalised global error of a field against a reference sampled at the same n points, Eq. 22:
+ *   E_phi = int (phi_0 - phi)^2 dV / int phi_0^2 dV = sum (ref - phi)^2 / sum ref^2   (uniform cells: dV cancels).
+ * A ratio of squares (no square root), not in percent; the paper's "phase field" is eta = sum_i eta_i.
+ * Returns -1.0 on bad arguments or a zero reference. */
+double pfo_error_eq22(long n, const double *phi, const double *ref);
 
 /* number of OpenMP threads the loops above will use (1 when built without -fopenmp). */
 int    pfo_num_threads(void);

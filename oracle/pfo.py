@@ -70,6 +70,8 @@ def lib():
         L.pfo_step_fd.argtypes = [pp, dp, dp, ctypes.c_int]
         L.pfo_free_energy.restype = ctypes.c_int
         L.pfo_free_energy.argtypes = [pp, dp, dp, ctypes.c_int, dp]
+        L.pfo_error_eq22.restype = ctypes.c_double
+        L.pfo_error_eq22.argtypes = [ctypes.c_long, dp, dp]
         L.pfo_num_threads.restype = ctypes.c_int
         L.pfo_num_threads.argtypes = []
         _lib = L
@@ -211,6 +213,18 @@ def fft1d_radix2(x: np.ndarray, sign: int = -1) -> np.ndarray:
     z = np.array(x, dtype=np.complex128, order="C")
     lib().pfo_fft1d_radix2(z.size, _dp(z.view(np.float64)), int(sign))
     return z
+
+
+def error_eq22(phi: np.ndarray, ref: np.ndarray) -> float:
+    """Eq. 22: sum (ref - phi)^2 / sum ref^2 over arrays sampled at the same points."""
+    a = np.ascontiguousarray(phi, dtype=np.float64).ravel()
+    b = np.ascontiguousarray(ref, dtype=np.float64).ravel()
+    if a.size != b.size:
+        raise ValueError("phi and ref must be sampled at the same points")
+    v = float(lib().pfo_error_eq22(a.size, _dp(a), _dp(b)))
+    if v < 0:
+        raise RuntimeError("pfo_error_eq22 failed (empty input or zero reference)")
+    return v
 
 
 def num_threads() -> int:

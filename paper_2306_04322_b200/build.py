@@ -9,6 +9,7 @@ paper_2306_04322_b200/libpf.so (static cudart; no torch, no other dependency).
 """
 from __future__ import annotations
 
+import glob
 import os
 import subprocess
 import sys
@@ -20,8 +21,7 @@ SUFFIX = os.environ.get("PF_BUILD_SUFFIX", "")
 OBJ = os.path.join(HERE, "csrc", "build" + ("_" + SUFFIX if SUFFIX else ""))
 SO = os.path.join(HERE, "libpf" + ("_" + SUFFIX if SUFFIX else "") + ".so")
 UNITS = ["row_kernels", "col_kernels", "fd_kernels", "pf"]
-HEADERS = [os.path.join(CSRC, h) for h in ("fft_core.cuh", "pf_kernels.cuh")] + \
-          [os.path.join(os.path.dirname(HERE), "include", "pf.h")]
+HEADERS = sorted(glob.glob(os.path.join(CSRC, "*.cuh"))) + [os.path.join(os.path.dirname(HERE), "include", "pf.h")]
 NVCC_FLAGS = ["-std=c++17", "-O3", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo",
               "-Xcompiler", "-fPIC", "-Xptxas", "-v"] + os.environ.get("PF_EXTRA_NVCC_FLAGS", "").split()
 

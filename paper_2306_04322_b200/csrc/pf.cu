@@ -23,7 +23,7 @@ using namespace pf;
 
 namespace {
 
-enum State { ST_NONE = 0, ST_REAL = 1, ST_SPECTRAL = 2, ST_BOTH = 3 };
+enum State { ST_NONE = 0, ST_REAL = 1, ST_SPECTRAL = 2, ST_BOTH = 3, ST_TIMING = 4 };
 const int kMaxFsKernels = 6;
 const int kProfBatch = 16;
 
@@ -34,6 +34,7 @@ struct pf_ctx {
     int F = 1, M = 0, P2 = 0;
     long N = 0;
     size_t w = 8;
+    int device = 0;                      // the CUDA device the context was created on (every call checks it is current)
     cudaStream_t stream = nullptr;
     bool own_stream = false;
     bool graph_ok = true;
@@ -51,7 +52,7 @@ struct pf_ctx {
     cudaGraphExec_t fs_graph = nullptr;
     int fs_graph_nodes = 0;
     // profiling
-    int profiling = 0;                   // 0 off; R >= 1: events around every kernel, each launched R times back to back
+    int profiling = 0;                   // events around every kernel of a step (no graph replay, no PDL)
     int nk = 0;
     const char *kname[kMaxFsKernels] = {};
     double kms[kMaxFsKernels] = {};
@@ -195,45 +196,55 @@ template <typename T> cudaError_t mid_forward(pf_ctx *c, const void *zsrc, long 
 
 // One FS step. 2D: x kernel, y kernel. 3D: x kernel, y-forward, z kernel, y-inverse. All launched with programmatic
 // stream serialization: each kernel's prologue overlaps its predecessor's tail (griddepcontrol in the kernels).
-template <typename T> int fs_one_step(pf_ctx *c, cudaEvent_t *events)
+// events != nullptr: one event after every kernel (profiling; launches are then kept strictly serial).
+// only >= 0: launch just that kernel of the step (timing aid, pf_launch_fs_kernel).
+template <typename T> int fs_one_step(pf_ctx *c, cudaEvent_t *events, int only = -1)
 {
-    const int rep = events ? (c->profiling > 1 ? c->profiling : 1) : 1;
     typedef typename V2<T>::type C;
     const int ny = c->p.n[1], nz = c->p.n[2];
     const long zfs = c->N / 2;
-    const bool pdl = events == nullptr;                 // timed launches are kept strictly serial
+    const bool pdl = events == nullptr && only < 0;
     KernelTimer kt(c, events);
-    RowParams<T> r = row_params<T>(c);
-    r.pdl = pdl;
-    for (int i = 0; i < rep; ++i) { PF_CK(c, launch_row<T>(ROW_STEP, c->p.n[0], r, c->stream)); ++c->launches; }
+    auto want = [&](int k) { return only < 0 || only == k; };
+    if (want(0)) {
+        RowParams<T> r = row_params<T>(c);
+        r.pdl = pdl;
+        PF_CK(c, launch_row<T>(ROW_STEP, c->p.n[0], r, c->stream)); ++c->launches;
+    }
     kt.mark("row_c2r_nonlinear_r2c");
     C *zst = (C *)c->zst;
     if (c->p.ndim == 2) {
-        ColParams<T> q = col_params<T>(c);
-        q.tw = (const C *)c->tw_y;
-        q.in_rs = q.out_rs = c->M;
-        q.in0 = zst; q.in1 = (const C *)c->zg; q.out = zst; q.in_fs = q.out_fs = zfs;
-        q.has_c = 1; q.pdl = pdl;
-        for (int i = 0; i < rep; ++i) { PF_CK(c, launch_col<T>(COL_2D_LAST, ny, c->F, 1, q, c->stream)); ++c->launches; }
+        if (want(1)) {
+            ColParams<T> q = col_params<T>(c);
+            q.tw = (const C *)c->tw_y;
+            q.in_rs = q.out_rs = c->M;
+            q.in0 = zst; q.in1 = (const C *)c->zg; q.out = zst; q.in_fs = q.out_fs = zfs;
+            q.has_c = 1; q.pdl = pdl;
+            PF_CK(c, launch_col<T>(COL_2D_LAST, ny, c->F, 1, q, c->stream)); ++c->launches;
+        }
         kt.mark("col_y_fft_update_ifft");
     } else {
         const long s2fs = (long)nz * ny * c->P2;
         C *s2 = (C *)c->s2;
-        for (int i = 0; i < rep; ++i) PF_CK(c, mid_forward<T>(c, zst, zfs, s2, s2fs, c->F, true, pdl));
+        if (want(1)) PF_CK(c, mid_forward<T>(c, zst, zfs, s2, s2fs, c->F, true, pdl));
         kt.mark("col_y_fwd");
-        ColParams<T> q = col_params<T>(c);
-        q.tw = (const C *)c->tw_z;
-        q.in_rs = q.out_rs = (long)ny * c->P2; q.ncols = ny * c->P2;
-        q.in0 = s2; q.in1 = (const C *)c->g2; q.out = s2; q.in_fs = q.out_fs = s2fs;
-        q.has_c = 1; q.pdl = pdl;
-        for (int i = 0; i < rep; ++i) { PF_CK(c, launch_col<T>(COL_3D_LAST, nz, c->F, 1, q, c->stream)); ++c->launches; }
+        if (want(2)) {
+            ColParams<T> q = col_params<T>(c);
+            q.tw = (const C *)c->tw_z;
+            q.in_rs = q.out_rs = (long)ny * c->P2; q.ncols = ny * c->P2;
+            q.in0 = s2; q.in1 = (const C *)c->g2; q.out = s2; q.in_fs = q.out_fs = s2fs;
+            q.has_c = 1; q.pdl = pdl;
+            PF_CK(c, launch_col<T>(COL_3D_LAST, nz, c->F, 1, q, c->stream)); ++c->launches;
+        }
         kt.mark("col_z_fft_update_ifft");
-        ColParams<T> v = col_params<T>(c);
-        v.tw = (const C *)c->tw_y;
-        v.in0 = s2; v.in_fs = s2fs; v.in_rs = c->P2; v.in_bs = (long)ny * c->P2;
-        v.out = zst; v.out_fs = zfs; v.out_rs = c->M; v.out_bs = (long)ny * c->M;
-        v.pdl = pdl;
-        for (int i = 0; i < rep; ++i) { PF_CK(c, launch_col<T>(COL_3D_MIDINV, ny, c->F, nz, v, c->stream)); ++c->launches; }
+        if (want(3)) {
+            ColParams<T> v = col_params<T>(c);
+            v.tw = (const C *)c->tw_y;
+            v.in0 = s2; v.in_fs = s2fs; v.in_rs = c->P2; v.in_bs = (long)ny * c->P2;
+            v.out = zst; v.out_fs = zfs; v.out_rs = c->M; v.out_bs = (long)ny * c->M;
+            v.pdl = pdl;
+            PF_CK(c, launch_col<T>(COL_3D_MIDINV, ny, c->F, nz, v, c->stream)); ++c->launches;
+        }
         kt.mark("col_y_inv");
     }
     c->nk = kt.k;
@@ -289,7 +300,7 @@ template <typename T> int step_fs(pf_ctx *c, int nsteps)
                     sum[k] += ms;
                 }
         }
-        for (int k = 0; k < c->nk; ++k) c->kms[k] = sum[k] / nsteps / (c->profiling > 1 ? c->profiling : 1);
+        for (int k = 0; k < c->nk; ++k) c->kms[k] = sum[k] / nsteps;
     } else {
         // replay one captured step; small grids are launch-latency bound without it
         if (!c->fs_graph && c->graph_ok) {
@@ -389,6 +400,13 @@ template <typename T> int free_energy(pf_ctx *c, int kind, double *out)
     return PF_OK;
 }
 
+// every entry point runs on the device the context was created on; a different current device is a caller error
+bool on_device(const pf_ctx *c)
+{
+    int d = -1;
+    return cudaGetDevice(&d) == cudaSuccess && d == c->device;
+}
+
 int copy_fields(pf_ctx *c, void *dc, void *deta, const void *sc, const void *seta, cudaMemcpyKind kind)
 {
     const size_t fb = (size_t)c->N * c->w;
@@ -441,12 +459,14 @@ int pf_create(const pf_params *p, pf_ctx **out)
     for (int d = 0; d < p->ndim; ++d) if (!pow2_in_range(p->n[d])) return PF_EUNSUPPORTED;
     if (p->ndim == 2 && p->n[2] != 1) return PF_EUNSUPPORTED;
 
-    int ndev = 0;
+    int ndev = 0, dev = 0;
     if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev <= 0) { cudaGetLastError(); return PF_ECUDA; }
+    if (cudaGetDevice(&dev) != cudaSuccess) { cudaGetLastError(); return PF_ECUDA; }
 
     pf_ctx *c = new (std::nothrow) pf_ctx();
     if (!c) return PF_ENOMEM;
     c->p = *p;
+    c->device = dev;
     if (p->ndim == 2) { c->p.n[2] = 1; c->p.dx[2] = 1.0; }
     c->F = 1 + p->n_eta;
     c->M = p->n[0] / 2;
@@ -488,6 +508,7 @@ int pf_set_fields(pf_ctx *c, const void *fc, const void *eta, int where)
 {
     if (!c || !fc || (c->p.n_eta > 0 && !eta)) return PF_EINVAL;
     if (where != PF_HOST && where != PF_DEVICE) return PF_EINVAL;
+    if (!on_device(c)) return PF_EINVAL;
     char *dst = (char *)c->real[c->cur];
     int rc = copy_fields(c, dst, dst + (size_t)c->N * c->w, fc, eta,
                          where == PF_HOST ? cudaMemcpyHostToDevice : cudaMemcpyDeviceToDevice);
@@ -502,7 +523,8 @@ int pf_get_fields(pf_ctx *c, void *fc, void *eta, int where)
 {
     if (!c || !fc || (c->p.n_eta > 0 && !eta)) return PF_EINVAL;
     if (where != PF_HOST && where != PF_DEVICE) return PF_EINVAL;
-    if (c->state == ST_NONE) return PF_ESTATE;
+    if (!on_device(c)) return PF_EINVAL;
+    if (c->state == ST_NONE || c->state == ST_TIMING) return PF_ESTATE;
     int rc = (c->p.precision == PF_F64) ? to_real<double>(c) : to_real<float>(c);
     if (rc) return rc;
     const char *src = (const char *)c->real[c->cur];
@@ -517,7 +539,8 @@ int pf_step_fs(pf_ctx *c, int nsteps)
 {
     if (!c || nsteps < 0) return PF_EINVAL;
     if (nsteps == 0) return PF_OK;
-    if (c->state == ST_NONE) return PF_ESTATE;
+    if (!on_device(c)) return PF_EINVAL;
+    if (c->state == ST_NONE || c->state == ST_TIMING) return PF_ESTATE;
     return (c->p.precision == PF_F64) ? step_fs<double>(c, nsteps) : step_fs<float>(c, nsteps);
 }
 
@@ -525,14 +548,16 @@ int pf_step_fd(pf_ctx *c, int nsteps)
 {
     if (!c || nsteps < 0) return PF_EINVAL;
     if (nsteps == 0) return PF_OK;
-    if (c->state == ST_NONE) return PF_ESTATE;
+    if (!on_device(c)) return PF_EINVAL;
+    if (c->state == ST_NONE || c->state == ST_TIMING) return PF_ESTATE;
     return (c->p.precision == PF_F64) ? step_fd<double>(c, nsteps) : step_fd<float>(c, nsteps);
 }
 
 int pf_free_energy(pf_ctx *c, int gradient_kind, double *out)
 {
     if (!c || !out || (gradient_kind != 0 && gradient_kind != 1)) return PF_EINVAL;
-    if (c->state == ST_NONE) return PF_ESTATE;
+    if (!on_device(c)) return PF_EINVAL;
+    if (c->state == ST_NONE || c->state == ST_TIMING) return PF_ESTATE;
     return (c->p.precision == PF_F64) ? free_energy<double>(c, gradient_kind, out)
                                       : free_energy<float>(c, gradient_kind, out);
 }
@@ -550,9 +575,23 @@ long long pf_launch_count(const pf_ctx *c) { return c ? c->launches : 0; }
 int pf_set_profiling(pf_ctx *c, int on)
 {
     if (!c) return PF_EINVAL;
-    c->profiling = on > 0 ? on : 0;
+    c->profiling = on > 0 ? 1 : 0;
     for (double &v : c->kms) v = -1.0;
     return PF_OK;
+}
+int pf_launch_fs_kernel(pf_ctx *c, int which)
+{
+    if (!c || which < 0 || which >= pf_num_fs_kernels(c)) return PF_EINVAL;
+    if (!on_device(c)) return PF_EINVAL;
+    if (c->state == ST_NONE) return PF_ESTATE;   /* ST_TIMING is fine here */
+    int rc = (c->p.precision == PF_F64) ? to_spectral<double>(c) : to_spectral<float>(c);
+    if (rc) return rc;
+    rc = (c->p.precision == PF_F64) ? fs_one_step<double>(c, nullptr, which) : fs_one_step<float>(c, nullptr, which);
+    // one kernel of a step applied on its own: the buffers are no trajectory any more. The context keeps serving
+    // further pf_launch_fs_kernel calls (timing), but stepping and read-out need pf_set_fields first.
+    c->state = ST_TIMING;
+    c->s2c_valid = true;
+    return rc;
 }
 int pf_num_fs_kernels(const pf_ctx *c)
 {
@@ -560,6 +599,12 @@ int pf_num_fs_kernels(const pf_ctx *c)
     return c->p.ndim == 2 ? 2 : 4;
 }
 double pf_fs_kernel_ms(pf_ctx *c, int which) { return (c && which >= 0 && which < c->nk) ? c->kms[which] : -1.0; }
-const char *pf_fs_kernel_name(const pf_ctx *c, int which) { return (c && which >= 0 && which < c->nk && c->kname[which]) ? c->kname[which] : ""; }
+const char *pf_fs_kernel_name(const pf_ctx *c, int which)
+{
+    static const char *k2d[] = {"row_c2r_nonlinear_r2c", "col_y_fft_update_ifft"};
+    static const char *k3d[] = {"row_c2r_nonlinear_r2c", "col_y_fwd", "col_z_fft_update_ifft", "col_y_inv"};
+    if (!c || which < 0 || which >= pf_num_fs_kernels(c)) return "";
+    return c->p.ndim == 2 ? k2d[which] : k3d[which];
+}
 
 }  // extern "C"

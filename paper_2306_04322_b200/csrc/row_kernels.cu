@@ -30,6 +30,9 @@
 #define PF_ROW_REGS_BIG 80
 #endif
 #define PF_ROW_REGS(T, M, E) ((((E) >= 16) && sizeof(T) == 8) ? 128 : ((M) >= 256) ? PF_ROW_REGS_BIG : 64)
+// fp64 rows of nx = 2048 with 7..9 fields: F * 128 threads at 80 registers do not fit an SM (register file, and 1152 >
+// 1024 threads at F = 9), so these run 16 elements per thread: F * 64 <= 576 threads under a 112-register cap
+#define PF_ROW_REGS_WIDE 112
 
 namespace pf {
 
@@ -57,8 +60,8 @@ template <int M, int E> __host__ __device__ constexpr int row_pitch() { return M
 // Register cap: the kernel is bound by fp64 issue and shared-memory exchange latency, so resident warps matter more
 // than the last few registers (measured on B200: 94 -> 80 registers: 1024^2 row kernel 28.1 -> 26.4 us; 64 at
 // nx = 256: 394 -> 317 us at 256^3).
-template <typename T, int M, int E, int MODE>
-__global__ void __maxnreg__(PF_ROW_REGS(T, M, E)) row_kernel(const RowParams<T> p)
+template <typename T, int M, int E, int MODE, int REGS>
+__global__ void __maxnreg__(REGS) row_kernel(const RowParams<T> p)
 {
 #ifdef PF_DBG_EMPTY
     return;
@@ -153,20 +156,20 @@ __global__ void __maxnreg__(PF_ROW_REGS(T, M, E)) row_kernel(const RowParams<T> 
     }
 }
 
-template <typename T, int M, int E, int MODE>
+template <typename T, int M, int E, int MODE, int REGS>
 static cudaError_t launch_row_inst(const RowParams<T> &p, cudaStream_t s)
 {
     typedef typename V2<T>::type C;
     constexpr int TT = M / E;
     const int per_row = TT * p.F;
-    if (per_row > 1024) return cudaErrorInvalidConfiguration;
+    if (per_row > 1024 || per_row * REGS > 65536) return cudaErrorInvalidConfiguration;
     int RB = PF_ROW_THREADS / per_row;
     if (RB > p.nrows / 296) RB = p.nrows / 296;      // small grids: at least two CTAs per SM before rows are batched
     if (RB < 1) RB = 1;
     if (RB > p.nrows) RB = p.nrows;
     const int threads = RB * per_row;
     const size_t smem = (size_t)RB * p.F * row_pitch<M, E>() * sizeof(C);
-    auto kern = row_kernel<T, M, E, MODE>;
+    auto kern = row_kernel<T, M, E, MODE, REGS>;
     if (smem > 48 * 1024) {
         cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
         if (e != cudaSuccess) return e;
@@ -175,13 +178,13 @@ static cudaError_t launch_row_inst(const RowParams<T> &p, cudaStream_t s)
     return launch_pdl(kern, dim3(grid), dim3(threads), smem, s, p.pdl != 0, p);
 }
 
-template <typename T, int M, int E>
+template <typename T, int M, int E, int REGS = PF_ROW_REGS(T, M, E)>
 static cudaError_t launch_row_mode(int mode, const RowParams<T> &p, cudaStream_t s)
 {
     switch (mode) {
-    case ROW_SET:  return launch_row_inst<T, M, E, ROW_SET>(p, s);
-    case ROW_STEP: return launch_row_inst<T, M, E, ROW_STEP>(p, s);
-    case ROW_GET:  return launch_row_inst<T, M, E, ROW_GET>(p, s);
+    case ROW_SET:  return launch_row_inst<T, M, E, ROW_SET, REGS>(p, s);
+    case ROW_STEP: return launch_row_inst<T, M, E, ROW_STEP, REGS>(p, s);
+    case ROW_GET:  return launch_row_inst<T, M, E, ROW_GET, REGS>(p, s);
     }
     return cudaErrorInvalidValue;
 }
@@ -197,7 +200,13 @@ template <typename T> cudaError_t launch_row(int mode, int nx, const RowParams<T
     case 256:  return launch_row_mode<T, 256, 8>(mode, p, s);
     case 512:  return launch_row_mode<T, 512, 8>(mode, p, s);
     // fp32 at nx = 2048: 16 elements per thread (the bytes an fp64 thread holds with 8), two CTAs per SM
-    case 1024: return (sizeof(T) == 4) ? launch_row_mode<T, 1024, 16>(mode, p, s) : launch_row_mode<T, 1024, PF_ROW_E1024>(mode, p, s);
+    case 1024:
+        if constexpr (sizeof(T) == 4) return launch_row_mode<T, 1024, 16>(mode, p, s);
+        else {
+            if (p.F * (1024 / PF_ROW_E1024) * PF_ROW_REGS(T, 1024, PF_ROW_E1024) > 65536)
+                return launch_row_mode<T, 1024, 16, PF_ROW_REGS_WIDE>(mode, p, s);
+            return launch_row_mode<T, 1024, PF_ROW_E1024>(mode, p, s);
+        }
     }
     return cudaErrorInvalidValue;
 }

@@ -20,7 +20,7 @@ PF_HOST, PF_DEVICE = 0, 1
 PF_OK, PF_EINVAL, PF_ENOMEM, PF_ECUDA, PF_ESTATE, PF_EUNSUPPORTED = 0, -1, -2, -3, -4, -5
 
 EXPORTS = ["pf_create", "pf_set_fields", "pf_step_fs", "pf_step_fd", "pf_get_fields", "pf_free_energy",
-           "pf_set_dt", "pf_launch_count", "pf_set_profiling", "pf_num_fs_kernels", "pf_fs_kernel_ms",
+           "pf_set_dt", "pf_launch_count", "pf_set_profiling", "pf_num_fs_kernels", "pf_fs_kernel_ms", "pf_launch_fs_kernel",
            "pf_fs_kernel_name", "pf_strerror", "pf_last_cuda_error", "pf_destroy"]
 
 
@@ -78,6 +78,8 @@ def lib() -> ctypes.CDLL:
         L.pf_fs_kernel_ms.argtypes = [vp, ctypes.c_int]
         L.pf_fs_kernel_name.restype = ctypes.c_char_p
         L.pf_fs_kernel_name.argtypes = [vp, ctypes.c_int]
+        L.pf_launch_fs_kernel.restype = ctypes.c_int
+        L.pf_launch_fs_kernel.argtypes = [vp, ctypes.c_int]
         L.pf_strerror.restype = ctypes.c_char_p
         L.pf_strerror.argtypes = [ctypes.c_int]
         L.pf_last_cuda_error.restype = ctypes.c_char_p
@@ -166,10 +168,16 @@ class Context:
     def launch_count(self) -> int:
         return int(lib().pf_launch_count(self._h))
 
-    def set_profiling(self, repeat):
-        """0/False: off; 1/True: events around every kernel; R > 1: every kernel launched R times between its events
-        (timing only: the fields are not a valid trajectory afterwards, see pf.h)."""
-        self._ck(lib().pf_set_profiling(self._h, int(repeat)), "pf_set_profiling")
+    def set_profiling(self, on):
+        """Events around every kernel of a step (no graph replay); see pf.h."""
+        self._ck(lib().pf_set_profiling(self._h, int(bool(on))), "pf_set_profiling")
+
+    def launch_fs_kernel(self, which: int):
+        """Timing aid (pf.h): queues only kernel `which` of a step; the fields are no trajectory afterwards."""
+        self._ck(lib().pf_launch_fs_kernel(self._h, int(which)), "pf_launch_fs_kernel")
+
+    def fs_kernel_names(self):
+        return [lib().pf_fs_kernel_name(self._h, i).decode() for i in range(lib().pf_num_fs_kernels(self._h))]
 
     def fs_kernel_times(self):
         """[(name, ms)] of the most recent profiled pf_step_fs call."""

@@ -91,3 +91,36 @@ def test_get_fields_twice_and_continue(oracle):
         gc, geta = ctx.get_fields()
     rc, reta = oracle.Model(n=n, n_eta=p, dx=dx, dt=5e-3).step_fs(c, eta, 7)
     assert rel_linf([gc, geta], [rc, reta]) < 1e-10
+
+
+def test_single_kernel_launches_leave_no_trajectory():
+    # pf_launch_fs_kernel is a timing aid (bench.py's per-kernel figures): afterwards the context must refuse to step or
+    # read out until fields are set again (a profiled context silently returned garbage)
+    n, p = (64, 32, 16), 2
+    c, eta, dx = synth.init_b(n, p)
+    with pf.Context(n, n_eta=p, dx=dx, dt=5e-3) as ctx:
+        with pytest.raises(pf.PfError) as e:
+            ctx.launch_fs_kernel(0)
+        assert e.value.code == pf.PF_ESTATE
+        ctx.set_fields(c, eta)
+        assert ctx.fs_kernel_names() == ["row_c2r_nonlinear_r2c", "col_y_fwd", "col_z_fft_update_ifft", "col_y_inv"]
+        l0 = ctx.launch_count()
+        for k in range(4):
+            ctx.launch_fs_kernel(k)
+            ctx.launch_fs_kernel(k)
+        assert ctx.launch_count() - l0 >= 8
+        with pytest.raises(pf.PfError) as e:
+            ctx.launch_fs_kernel(4)
+        assert e.value.code == pf.PF_EINVAL
+        for call in (lambda: ctx.step_fs(1), lambda: ctx.step_fd(1), ctx.get_fields, ctx.free_energy):
+            with pytest.raises(pf.PfError) as e:
+                call()
+            assert e.value.code == pf.PF_ESTATE
+        ctx.set_fields(c, eta)                           # and it recovers
+        ctx.step_fs(2)
+        a = ctx.get_fields()
+    with pf.Context(n, n_eta=p, dx=dx, dt=5e-3) as ctx:
+        ctx.set_fields(c, eta)
+        ctx.step_fs(2)
+        b = ctx.get_fields()
+    assert np.array_equal(a[0], b[0]) and np.array_equal(a[1], b[1])

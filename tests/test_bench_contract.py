@@ -31,3 +31,25 @@ def test_byte_model_matches_survey_8d():
         assert abs(sum(survey.values()) - expect) / expect < 1e-3
         assert sum(design.values()) < sum(survey.values())          # cross-step fusion moves fewer bytes than the per-pass ideal
         assert set(survey) == set(design)
+
+
+def test_gpus_flag_spawns_ranks_itself():
+    # `python bench.py --gpus 2` (no torchrun around it) must start two ranks; in the reference arm rank 0 alone works and
+    # prints, rank 1 exits 0 -> exactly one JSON line with n_gpus = 2
+    env = dict(os.environ)
+    for k in ("RANK", "WORLD_SIZE", "LOCAL_RANK"):
+        env.pop(k, None)
+    r = subprocess.run([sys.executable, os.path.join(ROOT, "bench.py"), "--gpus", "2", "--impl", "reference", "--workload", "64sq",
+                        "--steps", "2", "--warmup", "1"], capture_output=True, text=True, timeout=600, env=env)
+    assert r.returncode == 0, r.stderr[-2000:]
+    lines = [l for l in r.stdout.splitlines() if l.strip().startswith("{")]
+    assert len(lines) == 1
+    d = json.loads(lines[0])
+    assert d["impl"] == "reference" and d["n_gpus"] == 2
+
+
+def test_lib_override_is_refused():
+    env = dict(os.environ, PF_LIBPF="/nonexistent/libpf_nocomp.so")
+    r = subprocess.run([sys.executable, os.path.join(ROOT, "bench.py"), "--steps", "2"], capture_output=True, text=True,
+                       timeout=600, env=env)
+    assert r.returncode != 0 and "PF_LIBPF" in r.stderr

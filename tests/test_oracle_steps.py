@@ -260,3 +260,53 @@ def test_synth_generators_are_seeded_and_order_free():
     c, eta, dx = synth.init_b((32, 32), 4)
     assert c.shape == (32, 32) and eta.shape == (4, 32, 32) and dx == (6.25, 6.25)
     assert np.isclose(c[0, 0], 0.5 + 0.05 * 3) and eta.min() >= 0
+
+
+def test_free_energy_closed_forms_3d(oracle):
+    # the 3D terms of the gradient energy (the dzu term of kind 1, the kz^2 term of kind 0), anisotropic box:
+    # c = c0 + a cos(kz z) -> spectral: V kappa_c a^2 kz^2 / 4; forward differences: kz^2 -> 2 (1 - cos(kz dz)) / dz^2.
+    # A y-mode in eta_1 and an oblique (x, z) mode in eta_2 make sure no axis is mistaken for another.
+    nx, ny, nz = 16, 8, 32
+    lx, ly, lz = 10.0, 6.0, 14.0
+    dx = (lx / nx, ly / ny, lz / nz)
+    m = oracle.Model(n=(nx, ny, nz), n_eta=2, dx=dx)
+    V = lx * ly * lz
+    x = (np.arange(nx) * dx[0])[None, None, :] + np.zeros((nz, ny, nx))
+    y = (np.arange(ny) * dx[1])[None, :, None] + np.zeros((nz, ny, nx))
+    z = (np.arange(nz) * dx[2])[:, None, None] + np.zeros((nz, ny, nx))
+    kz, ky, kx = 2 * np.pi * 5 / lz, 2 * np.pi * 1 / ly, 2 * np.pi * 2 / lx
+    kz2 = 2 * np.pi * 3 / lz
+    c0, a, b1, b2 = 0.45, 0.07, 0.2, 0.1
+    c = c0 + a * np.cos(kz * z)
+    eta = np.stack([b1 * np.cos(ky * y), b2 * np.cos(kx * x + kz2 * z)])
+    F0 = m.free_energy(c, eta, 0)
+    assert np.isclose(F0[2], V * m.kappa_c * a * a * kz * kz / 4, rtol=1e-12)
+    assert np.isclose(F0[3], V * m.kappa_eta * b1 * b1 * ky * ky / 4, rtol=1e-12)
+    assert np.isclose(F0[4], V * m.kappa_eta * b2 * b2 * (kx * kx + kz2 * kz2) / 4, rtol=1e-12)
+    F1 = m.free_energy(c, eta, 1)
+    t = lambda k, d: 2 * (1 - np.cos(k * d)) / d ** 2
+    assert np.isclose(F1[2], V * m.kappa_c * a * a * t(kz, dx[2]) / 4, rtol=1e-12)
+    assert np.isclose(F1[3], V * m.kappa_eta * b1 * b1 * t(ky, dx[1]) / 4, rtol=1e-12)
+    assert np.isclose(F1[4], V * m.kappa_eta * b2 * b2 * (t(kx, dx[0]) + t(kz2, dx[2])) / 4, rtol=1e-12)
+    # FS-FD frequencies in the Parseval form (k2_kind 1 = Eq. 20) agree with the forward differences
+    m1 = oracle.Model(n=(nx, ny, nz), n_eta=2, dx=dx, k2_kind=1)
+    np.testing.assert_allclose(m1.free_energy(c, eta, 0)[2:], F1[2:], rtol=1e-12)
+
+
+def test_eq22_closed_forms(oracle):
+    # Eq. 22: ratio of squared L2 norms, no square root, no percent.
+    n = 64
+    x = 2 * np.pi * np.arange(n) / n
+    A, B, a0 = 0.3, 0.25, 0.5
+    # same mode, different amplitude: (A - B)^2 / A^2
+    assert np.isclose(oracle.error_eq22(B * np.cos(3 * x), A * np.cos(3 * x)), (A - B) ** 2 / A ** 2, rtol=1e-13)
+    # common mean, orthogonal modes: (A^2/2 + B^2/2) / (a0^2 + A^2/2); the reference (second argument) normalises
+    e = oracle.error_eq22(a0 + B * np.cos(5 * x), a0 + A * np.cos(3 * x))
+    assert np.isclose(e, (A * A / 2 + B * B / 2) / (a0 * a0 + A * A / 2), rtol=1e-13)
+    e_swapped = oracle.error_eq22(a0 + A * np.cos(3 * x), a0 + B * np.cos(5 * x))
+    assert np.isclose(e_swapped, (A * A / 2 + B * B / 2) / (a0 * a0 + B * B / 2), rtol=1e-13) and e_swapped != e
+    assert oracle.error_eq22(np.ones(5), np.ones(5)) == 0.0
+    # 2D arrays are flattened: a constant offset d against a unit reference -> d^2
+    assert np.isclose(oracle.error_eq22(np.full((4, 6), 1.1), np.ones((4, 6))), 0.01, rtol=1e-12)
+    with pytest.raises(RuntimeError):
+        oracle.error_eq22(np.ones(4), np.zeros(4))
