@@ -4,7 +4,7 @@
     PF_EXTRA_NVCC_FLAGS="-DPF_DBG_SKIP_COMPUTE" PF_BUILD_SUFFIX=nocomp python -m paper_2306_04322_b200.build
         -> libpf_nocomp.so beside libpf.so (an ablation / experiment build; load it with PF_LIBPF=<path>, see pf.py)
 
-The four translation units are compiled in parallel and linked into
+The translation units are compiled in parallel and linked into
 paper_2306_04322_b200/libpf.so (static cudart; no torch, no other dependency).
 """
 from __future__ import annotations
@@ -20,7 +20,7 @@ CSRC = os.path.join(HERE, "csrc")
 SUFFIX = os.environ.get("PF_BUILD_SUFFIX", "")
 OBJ = os.path.join(HERE, "csrc", "build" + ("_" + SUFFIX if SUFFIX else ""))
 SO = os.path.join(HERE, "libpf" + ("_" + SUFFIX if SUFFIX else "") + ".so")
-UNITS = ["row_kernels", "col_kernels", "fd_kernels", "pf"]
+UNITS = ["row_kernels", "col_kernels", "wcol_kernels", "fd_kernels", "pf"]
 HEADERS = sorted(glob.glob(os.path.join(CSRC, "*.cuh"))) + [os.path.join(os.path.dirname(HERE), "include", "pf.h")]
 NVCC_FLAGS = ["-std=c++17", "-O3", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo",
               "-Xcompiler", "-fPIC", "-Xptxas", "-v"] + os.environ.get("PF_EXTRA_NVCC_FLAGS", "").split()

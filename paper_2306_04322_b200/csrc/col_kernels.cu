@@ -24,6 +24,15 @@
 // what it wrote itself; the 8 MB stay in L2), then transform c^, combine, invert and store.
 #include "pf_kernels.cuh"
 #include "col_buf.cuh"
+#include "wfft.cuh"
+
+// -DPF_WFFT: long fp64 axes use the warp-tile transform of wfft.cuh (one shared-memory exchange per transform, the rest
+// in warp shuffles) instead of the Stockham path of fft_core.cuh. Measured on B200 and NOT the default: it removes 23 % of
+// the shared-memory wavefronts and two thirds of the barriers but adds 31 % instructions (the selects of the shuffle
+// transposes) and comes out level at 1024^2 and slower at 512^2 / 2048^2 (profiles/r2_col_variants.md)
+#ifndef PF_WFFT_MIN_N
+#define PF_WFFT_MIN_N 512
+#endif
 
 // column pairs per CTA at the longer axes (tuned on B200)
 #ifndef PF_COL_THREADS_PER_SM
@@ -80,6 +89,11 @@ template <int N, int E, int TP> struct ColShape {
     static constexpr int BUDGET = PF_COL_THREADS_PER_SM;                 // resident threads per SM the register cap is set for (1024: 64 registers)
     static constexpr int MINB = (THREADS >= BUDGET) ? 1 : ((BUDGET / THREADS > 32) ? 32 : BUDGET / THREADS);
     static constexpr int LR = (E >= 16) ? 4 : 3;                         // log2 of the first-stage radix
+#ifdef PF_WFFT
+    static constexpr bool WF = (E == 8 && TP == 2 && N >= PF_WFFT_MIN_N && N >= 256 && N <= 2048);
+#else
+    static constexpr bool WF = false;
+#endif
 };
 
 template <typename T, int N, int E, int TP, int MODE>
@@ -113,8 +127,25 @@ col_kernel(const ColParams<T> p)
     const int ub = blockIdx.x;                         // block of SLOTS columns
     const bool c_cta = DO_UPD && p.has_c && slot == 0;
 
+    constexpr bool WF = Sh::WF && sizeof(T) == 8;
     ColBuf<C, SLOTS, Sh::LR> buf{reinterpret_cast<C *>(smem_raw), sl};
     const CtaSync sync;
+    // warp-tile kernels keep the twiddle table and the |xi|^2 table of the FFT axis in shared memory behind the exchange
+    // buffer: every transform needs two twiddles and every update eight frequencies per thread, all of them scattered
+    // 8/16-byte reads that miss L1 (ncu: 42 % of the load requests and as many L2 sectors as the field data)
+    C *s_tw = reinterpret_cast<C *>(smem_raw) + (size_t)N * SLOTS;
+    T *s_k2 = reinterpret_cast<T *>(s_tw + N);
+#ifdef PF_NO_SMEM_TABLES
+    constexpr bool TS = false;
+#else
+    constexpr bool TS = WF;
+#endif
+    WFft<T, WF ? N : 1024, TS> wf(reinterpret_cast<C *>(smem_raw), TS ? s_tw : p.tw, tid);
+    // memory row and (after a forward transform) frequency index of register q
+    auto rowq = [&](int q) -> int { if constexpr (WF) return wf.row(q); else return j + q * TT; };
+    auto kq = [&](int q) -> int { if constexpr (WF) return wf.kidx(q); else return j + q * TT; };
+    auto forward = [&](C (&x)[E]) { if constexpr (WF) wf.dif(x); else fft_forward<N, E>(x, j, p.tw, buf, sync); };
+    auto transposed = [&](C (&x)[E]) { if constexpr (WF) wf.dit(x); else fft_forward<N, E>(x, j, p.tw, buf, sync); };
 
     // ---- which column ----
     bool valid = true;
@@ -157,42 +188,65 @@ col_kernel(const ColParams<T> p)
     out += bz * p.out_bs;
 
     C v[E];
+    auto unpack = [&](C za, C zb) -> C {
+        // E = (za + conj zb)/2, O = -(i/2)(za - conj zb)
+        const C e = mk<T>(T(0.5) * (za.x + zb.x), T(0.5) * (za.y - zb.y));
+        const C o = mk<T>(T(0.5) * (za.y + zb.y), T(-0.5) * (za.x - zb.x));
+        const C wo = cmul(wx, o);
+        return side ? cconj(csub(e, wo)) : cadd(e, wo);
+    };
     auto load_columns = [&](const C *src) {
-        if (PAIR_IN) {
+#ifdef PF_COL_OWNLOAD
+        constexpr bool OWN = WF;                 // A/B build (profiles/r2_col_variants.md): measured slower
+#else
+        constexpr bool OWN = false;
+#endif
+        if constexpr (PAIR_IN && OWN) {
+            // every thread loads ITS z column straight into v (eight independent 16-byte requests in flight, no landing
+            // registers) and takes the mirror column from the neighbouring lane
+            const C *mine = src + (side ? zcolB : zcolA);
+#pragma unroll
+            for (int q = 0; q < E; ++q) v[q] = mine[(long)rowq(q) * p.in_rs];
 #pragma unroll
             for (int q = 0; q < E; ++q) {
-                const long i = j + q * TT;
-                const C za = src[i * p.in_rs + zcolA], zb = src[i * p.in_rs + zcolB];
-                // E = (za + conj zb)/2, O = -(i/2)(za - conj zb)
-                const C e = mk<T>(T(0.5) * (za.x + zb.x), T(0.5) * (za.y - zb.y));
-                const C o = mk<T>(T(0.5) * (za.y + zb.y), T(-0.5) * (za.x - zb.x));
-                const C wo = cmul(wx, o);
-                v[q] = side ? cconj(csub(e, wo)) : cadd(e, wo);
+                const C pv = shfl_xor1(v[q]);
+                v[q] = side ? unpack(pv, v[q]) : unpack(v[q], pv);
+            }
+        } else if (PAIR_IN) {
+#pragma unroll
+            for (int q = 0; q < E; ++q) {
+                const long i = rowq(q);
+                v[q] = unpack(src[i * p.in_rs + zcolA], src[i * p.in_rs + zcolB]);
             }
         } else {
 #pragma unroll
-            for (int q = 0; q < E; ++q) v[q] = src[(long)(j + q * TT) * p.in_rs + pcol];
+            for (int q = 0; q < E; ++q) v[q] = src[(long)rowq(q) * p.in_rs + pcol];
         }
     };
 
+    const T *klast = LAST3D ? p.kz2 : p.ky2;
+    if constexpr (TS) {
+        for (int i = tid; i < N; i += GT) { s_tw[i] = p.tw[i]; s_k2[i] = klast[i]; }
+        klast = s_k2;
+        __syncthreads();
+    }
     grid_dependency_wait();                // everything above touches constant tables only
     grid_dependents_launch();
 
-    const T *klast = LAST3D ? p.kz2 : p.ky2;
     C *park = nullptr;
     if (c_cta) {
         // Cahn-Hilliard needs two transforms on the same columns: dt M |xi|^2 g^ is formed first and parked in
         // global memory (thread-linear: written and read back by the same thread, L2 resident), then c^ follows.
         park = p.park + ((bz * gridDim.x + ub) * (long)E) * GT + tid;
         load_columns(in);
-        fft_forward<N, E>(v, j, p.tw, buf, sync);
+        forward(v);
 #pragma unroll
-        for (int q = 0; q < E; ++q) park[(long)q * GT] = cscale(v[q], p.m.dtM * (base2 + klast[j + q * TT]));
+        for (int q = 0; q < E; ++q) park[(long)q * GT] = cscale(v[q], p.m.dtM * (base2 + klast[kq(q)]));
         in = p.in0 + bz * p.in_bs;
     }
 
     load_columns(in);
-    if (DO_FWD) fft_forward<N, E>(v, j, p.tw, buf, sync);
+    if (DO_FWD) forward(v);
 
 #ifndef PF_DBG_SKIP_UPDATE
     if (DO_UPD) {
@@ -200,7 +254,7 @@ col_kernel(const ColParams<T> p)
         if (c_cta) {
 #pragma unroll
             for (int q = 0; q < E; ++q) {
-                const T k2 = base2 + klast[j + q * TT];
+                const T k2 = base2 + klast[kq(q)];
                 const T d = s * rcp(T(1) + p.m.dtMkc * k2 * k2);
                 const C gq = park[(long)q * GT];
                 v[q] = mk<T>((v[q].x - gq.x) * d, (v[q].y - gq.y) * d);
@@ -208,7 +262,7 @@ col_kernel(const ColParams<T> p)
         } else {
 #pragma unroll
             for (int q = 0; q < E; ++q) {
-                const T k2 = base2 + klast[j + q * TT];
+                const T k2 = base2 + klast[kq(q)];
                 v[q] = cscale(v[q], s * rcp(T(1) + p.m.dtLke * k2));
             }
         }
@@ -222,7 +276,7 @@ col_kernel(const ColParams<T> p)
         if (store_ok && kx <= M) {
 #pragma unroll
             for (int q = 0; q < E; ++q)
-                acc += wgt * (double)(base2 + klast[j + q * TT]) * ((double)v[q].x * v[q].x + (double)v[q].y * v[q].y);
+                acc += wgt * (double)(base2 + klast[kq(q)]) * ((double)v[q].x * v[q].x + (double)v[q].y * v[q].y);
         }
         double *red = reinterpret_cast<double *>(smem_raw);      // off the hot path: plain serial reduction
         __syncthreads();
@@ -240,7 +294,7 @@ col_kernel(const ColParams<T> p)
         // inverse = swap re/im, forward, swap re/im (unnormalised; the update folds 1/N in)
 #pragma unroll
         for (int q = 0; q < E; ++q) v[q] = cswap(v[q]);
-        fft_forward<N, E>(v, j, p.tw, buf, sync);
+        transposed(v);
         const T s = DO_UPD ? T(1) : T(1) / T(N);
 #pragma unroll
         for (int q = 0; q < E; ++q) v[q] = mk<T>(v[q].y * s, v[q].x * s);
@@ -259,12 +313,12 @@ col_kernel(const ColParams<T> p)
             const C wo = mk<T>(T(0.5) * (ua.x - ubv.x), T(0.5) * (ua.y + ubv.y));
             const C io = cmul_pi(cmul(wxc, wo));
             const C z = side ? cconj(csub(e, io)) : cadd(e, io);
-            if (store_ok) dst[(long)(j + q * TT) * p.out_rs] = z;
+            if (store_ok) dst[(long)rowq(q) * p.out_rs] = z;
         }
     } else {
 #pragma unroll
         for (int q = 0; q < E; ++q)
-            if (store_ok) out[(long)(j + q * TT) * p.out_rs + pcol] = v[q];
+            if (store_ok) out[(long)rowq(q) * p.out_rs + pcol] = v[q];
     }
 }
 
@@ -276,6 +330,7 @@ static cudaError_t launch_col_inst(int nslots, int nbatch, const ColParams<T> &p
     constexpr bool PAIRS = (MODE == COL_2D_LAST || MODE == COL_3D_MIDFWD || MODE == COL_3D_MIDINV || MODE == COL_2D_ENERGY);
     const int gx = PAIRS ? (p.M / 2 + TP) / TP : p.ncols / Sh::SLOTS;    // blocks of SLOTS columns
     size_t smem = (size_t)N * Sh::SLOTS * sizeof(C);
+    if (Sh::WF && sizeof(T) == 8) smem += (size_t)N * (sizeof(C) + sizeof(T));                      // twiddle and |xi|^2 tables
     if (smem < (size_t)Sh::THREADS * sizeof(double)) smem = (size_t)Sh::THREADS * sizeof(double);   // energy reduction
     auto kern = col_kernel<T, N, E, TP, MODE>;
     if (smem > 48 * 1024) {

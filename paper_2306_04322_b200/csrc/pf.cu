@@ -11,6 +11,7 @@
 //   tables   twiddles exp(-2 pi i k/n) for M, ny, nz, nx; |xi_d|^2 per axis (Eq. 16-21)
 #include <cmath>
 #include <cstdio>
+#include <cstdlib>
 #include <cstring>
 #include <new>
 #include <string>
@@ -38,12 +39,14 @@ struct pf_ctx {
     cudaStream_t stream = nullptr;
     bool own_stream = false;
     bool graph_ok = true;
+    bool use_wcol = false;              // PF_WCOL=1 in the environment: the persistent pipelined strided kernel (A/B runs, profiles/)
     void *real[2] = {nullptr, nullptr};
     int cur = 0;
     void *zst = nullptr, *zg = nullptr, *s2 = nullptr, *g2 = nullptr, *park = nullptr;
     void *tw_m = nullptr, *tw_y = nullptr, *tw_z = nullptr, *tw_nx = nullptr;
     void *kx2 = nullptr, *ky2 = nullptr, *kz2 = nullptr;
     double *acc = nullptr;
+    int *queue = nullptr;               // work queue of the persistent strided kernel
     int state = ST_NONE;
     bool s2c_valid = false;
     long long launches = 0;
@@ -164,6 +167,7 @@ template <typename T> ColParams<T> col_params(pf_ctx *c)
     q.twx = (const C *)c->tw_nx;
     q.kx2 = (const T *)c->kx2; q.ky2 = (const T *)c->ky2; q.kz2 = (const T *)c->kz2;
     q.acc = c->acc;
+    q.queue = c->queue;
     q.park = (C *)c->park;
     q.m = make_model<T>(c->p);
     return q;
@@ -220,7 +224,9 @@ template <typename T> int fs_one_step(pf_ctx *c, cudaEvent_t *events, int only =
             q.in_rs = q.out_rs = c->M;
             q.in0 = zst; q.in1 = (const C *)c->zg; q.out = zst; q.in_fs = q.out_fs = zfs;
             q.has_c = 1; q.pdl = pdl;
-            PF_CK(c, launch_col<T>(COL_2D_LAST, ny, c->F, 1, q, c->stream)); ++c->launches;
+            cudaError_t e = c->use_wcol ? launch_wcol2d<T>(ny, c->F, q, c->stream) : cudaErrorNotSupported;
+            if (e == cudaErrorNotSupported) e = launch_col<T>(COL_2D_LAST, ny, c->F, 1, q, c->stream);
+            PF_CK(c, e); ++c->launches;
         }
         kt.mark("col_y_fft_update_ifft");
     } else {
@@ -441,7 +447,7 @@ void pf_destroy(pf_ctx *c)
     drop_graph(c);
     for (auto &e : c->pev) if (e) cudaEventDestroy(e);
     void *bufs[] = {c->real[0], c->real[1], c->zst, c->zg, c->s2, c->g2, c->park, c->tw_m, c->tw_y, c->tw_z,
-                    c->tw_nx, c->kx2, c->ky2, c->kz2, c->acc};
+                    c->tw_nx, c->kx2, c->ky2, c->kz2, c->acc, c->queue};
     for (void *b : bufs) if (b) cudaFree(b);
     if (c->own_stream) cudaStreamDestroy(c->stream);
     delete c;
@@ -467,6 +473,7 @@ int pf_create(const pf_params *p, pf_ctx **out)
     if (!c) return PF_ENOMEM;
     c->p = *p;
     c->device = dev;
+    { const char *e = getenv("PF_WCOL"); c->use_wcol = (e && e[0] == '1'); }
     if (p->ndim == 2) { c->p.n[2] = 1; c->p.dx[2] = 1.0; }
     c->F = 1 + p->n_eta;
     c->M = p->n[0] / 2;
@@ -491,7 +498,7 @@ int pf_create(const pf_params *p, pf_ctx **out)
     int rc;
     if ((rc = alloc(&c->real[0], fb * c->F)) || (rc = alloc(&c->real[1], fb * c->F)) ||
         (rc = alloc(&c->zst, fb * c->F)) || (rc = alloc(&c->zg, fb)) ||
-        (rc = alloc((void **)&c->acc, sizeof(double) * 32)) ||
+        (rc = alloc((void **)&c->acc, sizeof(double) * 32)) || (rc = alloc((void **)&c->queue, sizeof(int) * 4)) ||
         (rc = alloc(&c->park, (size_t)(c->P2 + 16) * c->p.n[1] * c->p.n[2] * 2 * c->w)))
         return fail(rc);
     if (p->ndim == 3) {

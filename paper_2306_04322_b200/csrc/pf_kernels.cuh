@@ -65,6 +65,7 @@ template <typename T> struct ColParams {
     const T *ky2;            // per ky (2D last: the FFT axis; 3D last: the middle axis)
     const T *kz2;            // per kz (3D last: the FFT axis)
     double  *acc;            // energy modes: accumulator (one double per field)
+    int     *queue;          // persistent kernels (wcol_kernels.cu): {next item, CTAs finished}, zero between launches
     Model<T> m;
 };
 
@@ -91,6 +92,8 @@ template <typename T> struct EnergyParams {
 // ---- launchers (defined in the .cu files; return cudaGetLastError()) ----
 template <typename T> cudaError_t launch_row(int mode, int nx, const RowParams<T> &p, cudaStream_t s);
 template <typename T> cudaError_t launch_col(int mode, int nfft, int nslots, int nbatch, const ColParams<T> &p, cudaStream_t s);
+// persistent pipelined form of COL_2D_LAST for long fp64 axes; cudaErrorNotSupported when the shape has none
+template <typename T> cudaError_t launch_wcol2d(int nfft, int nslots, const ColParams<T> &p, cudaStream_t s);
 template <typename T> cudaError_t launch_fd_fused2d(const FdParams<T> &p, cudaStream_t s);
 template <typename T> cudaError_t launch_fd_fused3d(const FdParams<T> &p, cudaStream_t s);
 template <typename T> cudaError_t launch_energy(const EnergyParams<T> &p, cudaStream_t s);

@@ -31,8 +31,9 @@
 #endif
 #define PF_ROW_REGS(T, M, E) ((((E) >= 16) && sizeof(T) == 8) ? 128 : ((M) >= 256) ? PF_ROW_REGS_BIG : 64)
 // fp64 rows of nx = 2048 with 7..9 fields: F * 128 threads at 80 registers do not fit an SM (register file, and 1152 >
-// 1024 threads at F = 9), so these run 16 elements per thread: F * 64 <= 576 threads under a 112-register cap
-#define PF_ROW_REGS_WIDE 112
+// 1024 threads at F = 9), so these run 16 elements per thread: F * 64 <= 576 threads = 18 warps, i.e. up to 5 warps on one
+// of the four 16 K-register sub-partitions -> at most 102 registers per thread
+#define PF_ROW_REGS_WIDE 96
 
 namespace pf {
 
@@ -162,7 +163,8 @@ static cudaError_t launch_row_inst(const RowParams<T> &p, cudaStream_t s)
     typedef typename V2<T>::type C;
     constexpr int TT = M / E;
     const int per_row = TT * p.F;
-    if (per_row > 1024 || per_row * REGS > 65536) return cudaErrorInvalidConfiguration;
+    // the warps of a CTA are dealt round-robin to four sub-partitions of 16 K registers each
+    if (per_row > 1024 || ((per_row / 32 + 3) / 4) * 32 * REGS > 16384) return cudaErrorInvalidConfiguration;
     int RB = PF_ROW_THREADS / per_row;
     if (RB > p.nrows / 296) RB = p.nrows / 296;      // small grids: at least two CTAs per SM before rows are batched
     if (RB < 1) RB = 1;
@@ -203,7 +205,7 @@ template <typename T> cudaError_t launch_row(int mode, int nx, const RowParams<T
     case 1024:
         if constexpr (sizeof(T) == 4) return launch_row_mode<T, 1024, 16>(mode, p, s);
         else {
-            if (p.F * (1024 / PF_ROW_E1024) * PF_ROW_REGS(T, 1024, PF_ROW_E1024) > 65536)
+            if (p.F * (1024 / PF_ROW_E1024) * PF_ROW_REGS(T, 1024, PF_ROW_E1024) > 65536)      // F >= 7
                 return launch_row_mode<T, 1024, 16, PF_ROW_REGS_WIDE>(mode, p, s);
             return launch_row_mode<T, 1024, PF_ROW_E1024>(mode, p, s);
         }
