@@ -116,6 +116,9 @@ col_kernel(const ColParams<T> p)
     constexpr bool LAST3D = (MODE == COL_3D_LAST || MODE == COL_3D_ENERGY);
     static_assert(GT % 32 == 0, "a CTA must be whole warps");
 
+#ifdef PF_TRACE
+    TraceScope trace(p.trace, 1 + MODE);
+#endif
     extern __shared__ __align__(16) unsigned char smem_raw[];
     const int tid = threadIdx.x;
     const int sl = tid % SLOTS;                        // column slot: side = sl & 1, pair t = sl >> 1
@@ -320,6 +323,9 @@ col_kernel(const ColParams<T> p)
         for (int q = 0; q < E; ++q)
             if (store_ok) out[(long)rowq(q) * p.out_rs + pcol] = v[q];
     }
+#ifdef PF_TRACE
+    trace.finish();
+#endif
 }
 
 template <typename T, int N, int E, int TP, int MODE>

@@ -117,7 +117,8 @@ template <int N, int E, int NS> struct StageShape {
     static constexpr int S = E / R;                   // butterflies per thread
     static constexpr int TT = N / E;
 };
-template <int N, int E, int NS, typename C>
+// TWS: tw points to shared memory (plain loads) instead of global memory (read-only path)
+template <int N, int E, int NS, typename C, bool TWS = false>
 PF_HD void stage_twiddles(C (&w1)[StageShape<N, E, NS>::S], int j, const C *__restrict__ tw)
 {
     typedef StageShape<N, E, NS> Sh;
@@ -126,7 +127,8 @@ PF_HD void stage_twiddles(C (&w1)[StageShape<N, E, NS>::S], int j, const C *__re
         for (int m = 0; m < Sh::S; ++m) {
             const int k = (j + m * Sh::TT) & (NS - 1);
 #if defined(__CUDA_ARCH__)
-            w1[m] = __ldg(tw + k * (N / (NS * Sh::R)));
+            if (TWS) w1[m] = tw[k * (N / (NS * Sh::R))];
+            else w1[m] = __ldg(tw + k * (N / (NS * Sh::R)));
 #else
             w1[m] = tw[k * (N / (NS * Sh::R))];
 #endif
@@ -208,36 +210,57 @@ PF_HD void exchange_load(C (&v)[E], int j, const Buf &buf)
 // store<N, E, NS>(v, j) (Stockham scatter of a non-final stage) and load<N, E>(v, j) (elements j + q*TT).
 // w1 = twiddles of the stage that starts at NS; those of the next stage are requested between the two barriers
 // of the exchange, when the data registers are dead and the table latency hides behind the barrier.
-template <int N, int E, int NS, typename C, typename Buf, typename Sync>
-__device__ __forceinline__ void fft_stages_w(C (&v)[E], int j, const C *__restrict__ tw, Buf &buf, const Sync &sync,
+//
+// Pol is the execution policy of the group of threads that carries the transform:
+//   barrier()        barrier over (at least) the TT threads that share `buf`;
+//   begin_compute()  called before the butterflies of every stage, end_compute() after the barrier that follows the
+//                    butterflies of every stage but the last (the caller keeps computing after the last stage and ends
+//                    the phase itself). No-ops except where thread groups of an SM take turns on the fp64 pipe
+//                    (col2d_kernels.cu).
+template <typename Sync> struct SyncOnly {
+    const Sync &sync;
+    __device__ __forceinline__ void barrier() const { sync(); }
+    __device__ __forceinline__ void begin_compute() const {}
+    __device__ __forceinline__ void end_compute() const {}
+};
+template <int N, int E, int NS, bool TWS, typename C, typename Buf, typename Pol>
+__device__ __forceinline__ void fft_stages_p(C (&v)[E], int j, const C *__restrict__ tw, Buf &buf, Pol &pol,
                                              const C (&w1)[StageShape<N, E, NS>::S])
 {
+    pol.begin_compute();
     stage_compute_w<N, E, NS>(v, w1);
     constexpr int R = stage_radix(N, E, NS);
     if constexpr (NS * R < N) {
         C w2[StageShape<N, E, NS * R>::S];
-        sync();                                   // every thread has taken its elements of the previous exchange
+        pol.barrier();                            // every thread has taken its elements of the previous exchange
+        pol.end_compute();
 #ifndef PF_DBG_SKIP_EXCHANGE
         buf.template store<N, E, NS>(v, j);
 #endif
 #ifndef PF_NO_TW_HOIST
-        stage_twiddles<N, E, NS * R>(w2, j, tw);
+        stage_twiddles<N, E, NS * R, C, TWS>(w2, j, tw);
 #endif
-        sync();
+        pol.barrier();
 #ifdef PF_NO_TW_HOIST
-        stage_twiddles<N, E, NS * R>(w2, j, tw);
+        stage_twiddles<N, E, NS * R, C, TWS>(w2, j, tw);
 #endif
 #ifndef PF_DBG_SKIP_EXCHANGE
         buf.template load<N, E>(v, j);
 #endif
-        fft_stages_w<N, E, NS * R>(v, j, tw, buf, sync, w2);
+        fft_stages_p<N, E, NS * R, TWS>(v, j, tw, buf, pol, w2);
     }
 }
-template <int N, int E, typename C, typename Buf, typename Sync>
-__device__ __forceinline__ void fft_forward(C (&v)[E], int j, const C *__restrict__ tw, Buf &buf, const Sync &sync)
+template <int N, int E, bool TWS = false, typename C, typename Buf, typename Pol>
+__device__ __forceinline__ void fft_forward_p(C (&v)[E], int j, const C *__restrict__ tw, Buf &buf, Pol &pol)
 {
     C w0[StageShape<N, E, 1>::S];                 // the first stage has no twiddles; never read
-    fft_stages_w<N, E, 1>(v, j, tw, buf, sync, w0);
+    fft_stages_p<N, E, 1, TWS>(v, j, tw, buf, pol, w0);
+}
+template <int N, int E, bool TWS = false, typename C, typename Buf, typename Sync>
+__device__ __forceinline__ void fft_forward(C (&v)[E], int j, const C *__restrict__ tw, Buf &buf, const Sync &sync)
+{
+    SyncOnly<Sync> pol{sync};
+    fft_forward_p<N, E, TWS>(v, j, tw, buf, pol);
 }
 template <int E, typename C> __device__ __forceinline__ void swap_all(C (&v)[E])
 {

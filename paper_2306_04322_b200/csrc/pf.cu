@@ -20,6 +20,10 @@
 #include "../../include/pf.h"
 #include "pf_kernels.cuh"
 
+namespace pf {
+void col2d_schedule(int nblk, int n_eta, int slots, int *grid_out, int *per_cta_out, std::vector<int> &sched);
+void col2d_schedule_init(int nblk, int slots, int *grid_out, int *per_cta_out, std::vector<int> &sched);
+}
 using namespace pf;
 
 namespace {
@@ -27,6 +31,7 @@ namespace {
 enum State { ST_NONE = 0, ST_REAL = 1, ST_SPECTRAL = 2, ST_BOTH = 3, ST_TIMING = 4 };
 const int kMaxFsKernels = 6;
 const int kProfBatch = 16;
+const int kGraphSteps = 8;              // steps per captured graph (pf_step_fs calls of at least this many steps)
 
 }  // namespace
 
@@ -49,6 +54,14 @@ struct pf_ctx {
     int *queue = nullptr;               // work queue of the persistent strided kernel
     int state = ST_NONE;
     bool s2c_valid = false;
+    // 2D: carried spectrum of c and the static schedule of the last-axis kernel (col2d_kernels.cu)
+    bool legacy_col2d = false;           // PF_COL2D_LEGACY=1: the one-CTA-per-(field, block) kernel of col_kernels.cu (A/B runs)
+    void *carry = nullptr;
+    bool carry_valid = false;
+    int *c2_sched = nullptr, *c2_sched_init = nullptr, *c2_flags = nullptr;
+    int c2_grid = 0, c2_per = 0, c2_grid_init = 0, c2_per_init = 0;
+    int carveout = 0;                    // shared-memory carve-out both kernels of a 2D step run with (percent; 0: unset)
+    TraceBuf *trace = nullptr;           // -DPF_TRACE builds only
     long long launches = 0;
     std::string cuda_err;
     // CUDA graph of one FS step
@@ -154,7 +167,11 @@ template <typename T> RowParams<T> row_params(pf_ctx *c)
     r.tw = (const C *)c->tw_m;
     r.zfs = c->N / 2; r.rfs = c->N;
     r.nrows = c->p.n[1] * c->p.n[2]; r.F = c->F;
+    r.carveout = c->carveout;
     r.m = make_model<T>(c->p);
+#ifdef PF_TRACE
+    r.trace = c->trace;
+#endif
     return r;
 }
 
@@ -170,6 +187,29 @@ template <typename T> ColParams<T> col_params(pf_ctx *c)
     q.queue = c->queue;
     q.park = (C *)c->park;
     q.m = make_model<T>(c->p);
+#ifdef PF_TRACE
+    q.trace = c->trace;
+#endif
+    return q;
+}
+
+template <typename T> Col2dParams<T> col2d_params(pf_ctx *c, bool init, bool pdl)
+{
+    typedef typename V2<T>::type C;
+    Col2dParams<T> q;
+    memset(&q, 0, sizeof(q));
+    q.zst = (C *)c->zst; q.zg = (const C *)c->zg; q.carry = (C *)c->carry;
+    q.zfs = c->N / 2; q.M = c->M;
+    q.sched = init ? c->c2_sched_init : c->c2_sched;
+    q.per_cta = init ? c->c2_per_init : c->c2_per;
+    q.flags = c->c2_flags;
+    q.pdl = pdl;
+    q.tw = (const C *)c->tw_y; q.twx = (const C *)c->tw_nx;
+    q.kx2 = (const T *)c->kx2; q.ky2 = (const T *)c->ky2;
+    q.m = make_model<T>(c->p);
+#ifdef PF_TRACE
+    q.trace = c->trace;
+#endif
     return q;
 }
 
@@ -224,7 +264,9 @@ template <typename T> int fs_one_step(pf_ctx *c, cudaEvent_t *events, int only =
             q.in_rs = q.out_rs = c->M;
             q.in0 = zst; q.in1 = (const C *)c->zg; q.out = zst; q.in_fs = q.out_fs = zfs;
             q.has_c = 1; q.pdl = pdl;
-            cudaError_t e = c->use_wcol ? launch_wcol2d<T>(ny, c->F, q, c->stream) : cudaErrorNotSupported;
+            cudaError_t e = cudaErrorNotSupported;
+            if (c->use_wcol) e = launch_wcol2d<T>(ny, c->F, q, c->stream);
+            else if (!c->legacy_col2d) e = launch_col2d<T>(ny, col2d_params<T>(c, false, pdl), c->c2_grid, c->stream);
             if (e == cudaErrorNotSupported) e = launch_col<T>(COL_2D_LAST, ny, c->F, 1, q, c->stream);
             PF_CK(c, e); ++c->launches;
         }
@@ -264,6 +306,10 @@ template <typename T> int to_spectral(pf_ctx *c)
         RowParams<T> r = row_params<T>(c);
         PF_CK(c, launch_row<T>(ROW_SET, c->p.n[0], r, c->stream)); ++c->launches;
         c->state = ST_BOTH;
+    }
+    if (c->p.ndim == 2 && c->carry && !c->carry_valid) {
+        PF_CK(c, launch_col2d<T>(c->p.n[1], col2d_params<T>(c, true, false), c->c2_grid_init, c->stream)); ++c->launches;
+        c->carry_valid = true;
     }
     if (c->p.ndim == 3 && !c->s2c_valid) {
         PF_CK(c, mid_forward<T>(c, c->zst, 0, c->s2, 0, 1, false, false));
@@ -308,12 +354,15 @@ template <typename T> int step_fs(pf_ctx *c, int nsteps)
         }
         for (int k = 0; k < c->nk; ++k) c->kms[k] = sum[k] / nsteps;
     } else {
-        // replay one captured step; small grids are launch-latency bound without it
-        if (!c->fs_graph && c->graph_ok) {
+        // Every kernel is launched with programmatic stream serialization, so a kernel's CTAs become resident under its
+        // predecessor's last CTAs. Long runs replay a captured graph of kGraphSteps steps (the programmatic edges between
+        // ALL its kernels are kept; a graph of one step would serialise at every step boundary: 2.9 us of 52 at 1024^2,
+        // profiles/r2_col2d.md); what is left, and short calls, are plain launches.
+        if (!c->fs_graph && c->graph_ok && nsteps >= kGraphSteps) {
             cudaGraph_t g = nullptr;
             const long long before = c->launches;
             if (cudaStreamBeginCapture(c->stream, cudaStreamCaptureModeThreadLocal) == cudaSuccess) {
-                rc = fs_one_step<T>(c, nullptr);
+                for (int s = 0; s < kGraphSteps && !rc; ++s) rc = fs_one_step<T>(c, nullptr);
                 cudaError_t e = cudaStreamEndCapture(c->stream, &g);
                 c->fs_graph_nodes = (int)(c->launches - before);
                 c->launches = before;
@@ -327,10 +376,13 @@ template <typename T> int step_fs(pf_ctx *c, int nsteps)
                 c->graph_ok = false;
             }
         }
-        for (int s = 0; s < nsteps; ++s) {
-            if (c->fs_graph) { PF_CK(c, cudaGraphLaunch(c->fs_graph, c->stream)); c->launches += c->fs_graph_nodes; }
-            else if ((rc = fs_one_step<T>(c, nullptr))) return rc;
+        int left = nsteps;
+        for (; c->fs_graph && left >= kGraphSteps; left -= kGraphSteps) {
+            PF_CK(c, cudaGraphLaunch(c->fs_graph, c->stream));
+            c->launches += c->fs_graph_nodes;
         }
+        for (; left > 0; --left)
+            if ((rc = fs_one_step<T>(c, nullptr))) return rc;
     }
     c->state = ST_SPECTRAL;
     return PF_OK;
@@ -358,6 +410,7 @@ template <typename T> int step_fd(pf_ctx *c, int nsteps)
     }
     c->state = ST_REAL;
     c->s2c_valid = false;
+    c->carry_valid = false;
     return PF_OK;
 }
 
@@ -445,9 +498,24 @@ void pf_destroy(pf_ctx *c)
 {
     if (!c) return;
     drop_graph(c);
+#ifdef PF_TRACE
+    if (c->trace) {
+        cudaDeviceSynchronize();
+        const char *fn = getenv("PF_TRACE_FILE");
+        if (FILE *fh = fn ? fopen(fn, "a") : nullptr) {
+            const unsigned long long n = c->trace->n < c->trace->cap ? c->trace->n : c->trace->cap;
+            for (unsigned long long i = 0; i < n; ++i)
+                fprintf(fh, "%llu %llu %llu %llu\n", c->trace->rec[3 * i] >> 32, c->trace->rec[3 * i] & 0xffffffffull,
+                        c->trace->rec[3 * i + 1], c->trace->rec[3 * i + 2]);
+            fclose(fh);
+        }
+        cudaFree(c->trace);
+    }
+#endif
     for (auto &e : c->pev) if (e) cudaEventDestroy(e);
     void *bufs[] = {c->real[0], c->real[1], c->zst, c->zg, c->s2, c->g2, c->park, c->tw_m, c->tw_y, c->tw_z,
-                    c->tw_nx, c->kx2, c->ky2, c->kz2, c->acc, c->queue};
+                    c->tw_nx, c->kx2, c->ky2, c->kz2, c->acc, c->queue, c->carry, c->c2_sched, c->c2_sched_init,
+                    c->c2_flags};
     for (void *b : bufs) if (b) cudaFree(b);
     if (c->own_stream) cudaStreamDestroy(c->stream);
     delete c;
@@ -474,6 +542,8 @@ int pf_create(const pf_params *p, pf_ctx **out)
     c->p = *p;
     c->device = dev;
     { const char *e = getenv("PF_WCOL"); c->use_wcol = (e && e[0] == '1'); }
+    { const char *e = getenv("PF_COL2D_LEGACY"); c->legacy_col2d = (e && e[0] == '1'); }
+    { const char *e = getenv("PF_NO_GRAPH"); if (e && e[0] == '1') c->graph_ok = false; }
     if (p->ndim == 2) { c->p.n[2] = 1; c->p.dx[2] = 1.0; }
     c->F = 1 + p->n_eta;
     c->M = p->n[0] / 2;
@@ -507,6 +577,33 @@ int pf_create(const pf_params *p, pf_ctx **out)
     }
     rc = (p->precision == PF_F64) ? upload_tables<double>(c) : upload_tables<float>(c);
     if (rc) return fail(rc);
+    if (p->ndim == 2 && !c->legacy_col2d && !c->use_wcol) {
+        Col2dShapeInfo si;
+        cudaError_t e = (p->precision == PF_F64) ? col2d_shape<double>(c->p.n[1], c->M, &si) : col2d_shape<float>(c->p.n[1], c->M, &si);
+        if (e != cudaSuccess) { c->cuda_err = cudaGetErrorString(e); cudaGetLastError(); return fail(PF_ECUDA); }
+        c->carveout = si.carveout_pct;
+        std::vector<int> sched, sched_init;
+        col2d_schedule(si.nblk, p->n_eta, si.slots, &c->c2_grid, &c->c2_per, sched);
+        col2d_schedule_init(si.nblk, si.slots, &c->c2_grid_init, &c->c2_per_init, sched_init);
+        if ((rc = alloc(&c->carry, (size_t)si.carry_elems * 2 * c->w)) ||
+            (rc = alloc((void **)&c->c2_sched, sizeof(int) * sched.size())) ||
+            (rc = alloc((void **)&c->c2_sched_init, sizeof(int) * sched_init.size())) ||
+            (rc = alloc((void **)&c->c2_flags, sizeof(int) * (size_t)si.nblk)))
+            return fail(rc);
+        if (cudaMemcpy(c->c2_sched, sched.data(), sizeof(int) * sched.size(), cudaMemcpyHostToDevice) != cudaSuccess ||
+            cudaMemcpy(c->c2_sched_init, sched_init.data(), sizeof(int) * sched_init.size(), cudaMemcpyHostToDevice) != cudaSuccess) {
+            cudaGetLastError();
+            return fail(PF_ECUDA);
+        }
+    }
+#ifdef PF_TRACE
+    if (getenv("PF_TRACE_FILE")) {
+        const unsigned long long cap = 1ull << 20;
+        if (cudaMallocManaged((void **)&c->trace, sizeof(TraceBuf) + 3 * cap * sizeof(unsigned long long)) == cudaSuccess) {
+            c->trace->n = 0; c->trace->cap = cap;
+        } else { cudaGetLastError(); c->trace = nullptr; }
+    }
+#endif
     *out = c;
     return PF_OK;
 }
@@ -523,6 +620,7 @@ int pf_set_fields(pf_ctx *c, const void *fc, const void *eta, int where)
     if (where == PF_HOST) PF_CK(c, cudaStreamSynchronize(c->stream));
     c->state = ST_REAL;
     c->s2c_valid = false;
+    c->carry_valid = false;
     return PF_OK;
 }
 

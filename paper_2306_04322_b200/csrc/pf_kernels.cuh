@@ -16,6 +16,35 @@ template <typename T> struct Model {
     int n_eta;
 };
 
+// -DPF_TRACE builds (profiles/: CTA timelines): every CTA of the step kernels appends {kind, %smid, start, end} (%globaltimer,
+// ns) to a buffer the context dumps at pf_destroy into the file named by PF_TRACE_FILE. Never part of the default library.
+struct TraceBuf { unsigned long long n, cap; unsigned long long rec[1]; };
+#if defined(PF_TRACE) && defined(__CUDACC__)
+#define PF_TRACE_FIELD TraceBuf *trace;
+struct TraceScope {
+    TraceBuf *b; unsigned long long t0; int kind;
+    __device__ __forceinline__ TraceScope(TraceBuf *buf, int k) : b(buf), kind(k)
+    {
+        asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t0));
+    }
+    __device__ __forceinline__ void finish()
+    {
+        __syncthreads();
+        if (b && threadIdx.x == 0) {
+            unsigned long long t1; unsigned sm;
+            asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t1));
+            asm volatile("mov.u32 %0, %%smid;" : "=r"(sm));
+            const unsigned long long i = atomicAdd(&b->n, 1ull);
+            if (i < b->cap) { b->rec[3 * i] = ((unsigned long long)kind << 32) | sm; b->rec[3 * i + 1] = t0; b->rec[3 * i + 2] = t1; }
+        }
+    }
+};
+#elif defined(PF_TRACE)
+#define PF_TRACE_FIELD TraceBuf *trace;
+#else
+#define PF_TRACE_FIELD
+#endif
+
 enum RowMode { ROW_SET = 0, ROW_STEP = 1, ROW_GET = 2 };
 
 // x-direction kernel. "z-form" of a real row u[0..nx): Z = FFT_{nx/2}( u[2n] + i u[2n+1] ), nx/2 complex values.
@@ -30,7 +59,9 @@ template <typename T> struct RowParams {
     int      nrows;          // ny*nz
     int      F;              // 1 + n_eta
     int      pdl;            // launch with programmatic stream serialization
+    int      carveout;       // preferred shared-memory carve-out in percent (0: the driver's choice), see col2d_shape()
     Model<T> m;
+    PF_TRACE_FIELD
 };
 
 // Column-kernel modes (see col_kernels.cu)
@@ -67,7 +98,38 @@ template <typename T> struct ColParams {
     double  *acc;            // energy modes: accumulator (one double per field)
     int     *queue;          // persistent kernels (wcol_kernels.cu): {next item, CTAs finished}, zero between launches
     Model<T> m;
+    PF_TRACE_FIELD
 };
+
+// 2D last-axis kernel with carried c^ and a static balanced schedule (col2d_kernels.cu)
+enum Col2dOp {
+    COL2D_ETA    = 0,   // Allen-Cahn block: unpack, FFT_y, Eq. 15, IFFT_y, repack                       (two rounds)
+    COL2D_C_FWD  = 1,   // Cahn-Hilliard block, first half: unpack g, FFT_y, Eq. 14 on the carried c^    (one round)
+    COL2D_C_INV  = 2,   // second half: carried c^ -> IFFT_y, repack                                     (one round)
+    COL2D_C_FULL = 3,   // both halves in one CTA, values kept in registers
+    COL2D_C_INIT = 4    // z-form of c -> unpack, FFT_y -> carry (after pf_set_fields / FD steps)
+};
+template <typename T> struct Col2dParams {
+    typedef typename V2<T>::type C;
+    C       *zst;            // [F][ny][M] z-form state; slot s at zst + s*zfs (slot 0 = c, written by C_INV / C_FULL)
+    const C *zg;             // [ny][M] z-form of g = df/dc
+    C       *carry;          // c^ in the kernel's thread-linear order: [nblk][E][THREADS]
+    long     zfs;
+    int      M;              // nx/2 = pitch of the z-form rows
+    int      per_cta;        // items per CTA in sched (padded with -1; at most Col2dShapeInfo::max_items)
+    const int *sched;        // [grid][per_cta] items: op | slot << 4 | block << 8
+    int     *flags;          // [nblk] C_FWD -> C_INV hand-off, zero between launches
+    int      pdl;
+    const C *tw;             // exp(-2 pi i k / ny)
+    const C *twx;            // exp(-2 pi i k / nx), k <= M/2
+    const T *kx2, *ky2;      // |xi_x|^2 per kx (M+1 entries), |xi_y|^2 per ky
+    Model<T> m;
+    PF_TRACE_FIELD
+};
+// carveout_pct: the shared-memory carve-out (percent of the SM's maximum) the kernel runs with. An SM switches carve-out
+// only when it is idle, so a kernel launched with programmatic stream serialization becomes resident under its
+// predecessor's last CTAs only if both run with the SAME carve-out: the x kernel is given this value too.
+struct Col2dShapeInfo { int tp, e, threads, max_items, nblk, slots, carveout_pct; long carry_elems; };
 
 // FD path
 template <typename T> struct FdParams {
@@ -94,6 +156,8 @@ template <typename T> cudaError_t launch_row(int mode, int nx, const RowParams<T
 template <typename T> cudaError_t launch_col(int mode, int nfft, int nslots, int nbatch, const ColParams<T> &p, cudaStream_t s);
 // persistent pipelined form of COL_2D_LAST for long fp64 axes; cudaErrorNotSupported when the shape has none
 template <typename T> cudaError_t launch_wcol2d(int nfft, int nslots, const ColParams<T> &p, cudaStream_t s);
+template <typename T> cudaError_t col2d_shape(int nfft, int M, Col2dShapeInfo *o);
+template <typename T> cudaError_t launch_col2d(int nfft, const Col2dParams<T> &p, int grid, cudaStream_t s);
 template <typename T> cudaError_t launch_fd_fused2d(const FdParams<T> &p, cudaStream_t s);
 template <typename T> cudaError_t launch_fd_fused3d(const FdParams<T> &p, cudaStream_t s);
 template <typename T> cudaError_t launch_energy(const EnergyParams<T> &p, cudaStream_t s);

@@ -70,6 +70,9 @@ __global__ void __maxnreg__(REGS) row_kernel(const RowParams<T> p)
     typedef typename V2<T>::type C;
     constexpr int TT = M / E;
     constexpr int MP = row_pitch<M, E>();
+#ifdef PF_TRACE
+    TraceScope trace(p.trace, 0);
+#endif
     extern __shared__ __align__(16) unsigned char smem_raw[];
     C *smem = reinterpret_cast<C *>(smem_raw);
 
@@ -155,6 +158,9 @@ __global__ void __maxnreg__(REGS) row_kernel(const RowParams<T> p)
 #pragma unroll
         for (int q = 0; q < E; ++q) dst[j + q * TT] = v[q];
     }
+#ifdef PF_TRACE
+    if (MODE == ROW_STEP) trace.finish();
+#endif
 }
 
 template <typename T, int M, int E, int MODE, int REGS>
@@ -174,6 +180,10 @@ static cudaError_t launch_row_inst(const RowParams<T> &p, cudaStream_t s)
     auto kern = row_kernel<T, M, E, MODE, REGS>;
     if (smem > 48 * 1024) {
         cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        if (e != cudaSuccess) return e;
+    }
+    if (p.carveout > 0) {
+        cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributePreferredSharedMemoryCarveout, p.carveout);
         if (e != cudaSuccess) return e;
     }
     const unsigned grid = (unsigned)((p.nrows + RB - 1) / RB);
