@@ -112,6 +112,10 @@ template <typename T> Model<T> make_model(const pf_params &p)
     m.dt = (T)p.dt; m.M = (T)p.M; m.L = (T)p.L;
     m.dtM = (T)(p.dt * p.M); m.dtL = (T)(p.dt * p.L);
     m.dtMkc = (T)(p.dt * p.M * p.kappa_c); m.dtLke = (T)(p.dt * p.L * p.kappa_eta);
+    m.gA0 = (T)(2.0 * p.rho2); m.gA1 = (T)(2.0 * p.rho2 * p.c_alpha); m.gA2 = (T)(2.0 * p.rho2 * (p.c_beta - p.c_alpha));
+    m.eB0 = (T)(30.0 * p.rho2 * (p.c_beta * p.c_beta - p.c_alpha * p.c_alpha));
+    m.eB1 = (T)(60.0 * p.rho2 * (p.c_beta - p.c_alpha));
+    m.eW2 = (T)(2.0 * p.w); m.eW4a = (T)(4.0 * p.alpha * p.w);
     m.n_eta = p.n_eta;
     return m;
 }

@@ -13,6 +13,10 @@ template <typename T> struct Model {
     T dt, M, L;
     T dtM, dtL;                            // dt*M, dt*L            (Eqs. 12-13)
     T dtMkc, dtLke;                        // dt*M*kappa_c, dt*L*kappa_eta   (Eqs. 14-15)
+    // derived constants of the pointwise derivatives (dfdc, dfdeta below), formed once on the host in double
+    T gA0, gA1, gA2;                       // df/dc = gA0 c - gA1 - gA2 h:  2 rho2, 2 rho2 c_alpha, 2 rho2 (c_beta - c_alpha)
+    T eB0, eB1;                            // 30 (f^beta - f^alpha) = eB0 - eB1 c:  30 rho2 (c_beta^2 - c_alpha^2), 60 rho2 (c_beta - c_alpha)
+    T eW2, eW4a;                           // 2 w, 4 alpha w
     int n_eta;
 };
 
@@ -214,21 +218,21 @@ static inline cudaError_t launch_pdl(K kern, dim3 grid, dim3 block, size_t smem,
 // h(eta) = sum eta^3 (6 eta^2 - 15 eta + 10); g(eta) = sum eta^2 (1-eta)^2 + alpha sum_i sum_{j!=i} eta_i^2 eta_j^2
 // f_chem = rho2 (c-c_alpha)^2 (1-h) + rho2 (c_beta-c)^2 h + w g
 template <typename T> PF_HD T h_term(T e) { return e * e * e * (e * (T(6) * e - T(15)) + T(10)); }
-// d f_chem / dc = 2 rho2 [ (c - c_alpha)(1 - h) - (c_beta - c) h ]
+// d f_chem / dc = 2 rho2 [ (c - c_alpha)(1 - h) - (c_beta - c) h ] = 2 rho2 (c - c_alpha) - 2 rho2 (c_beta - c_alpha) h
 template <typename T> PF_HD T dfdc(const Model<T> &m, T c, T h)
 {
-    return T(2) * m.rho2 * ((c - m.c_alpha) * (T(1) - h) - (m.c_beta - c) * h);
+    return (m.gA0 * c - m.gA1) - m.gA2 * h;
 }
 // d f_chem / d eta_i = (f^beta - f^alpha) 30 eta^2 (1-eta)^2 + w [ 2 eta (1-eta)(1-2 eta) + 4 alpha eta (s2 - eta^2) ],
-// s2 = sum_j eta_j^2 (each unordered pair appears twice in the ordered double sum of g -> 4 alpha)
+// s2 = sum_j eta_j^2 (each unordered pair appears twice in the ordered double sum of g -> 4 alpha);
+// f^beta - f^alpha = rho2 [(c_beta - c)^2 - (c - c_alpha)^2] = rho2 (c_beta - c_alpha)(c_beta + c_alpha - 2 c) is linear in c
 template <typename T> PF_HD T dfdeta(const Model<T> &m, T c, T e, T s2)
 {
-    const T da = c - m.c_alpha, db = m.c_beta - c;
-    const T fba = m.rho2 * (db * db - da * da);
-    const T ome = T(1) - e;
-    const T dh = T(30) * e * e * ome * ome;
-    const T dg = T(2) * e * ome * (T(1) - T(2) * e) + T(4) * m.alpha * e * (s2 - e * e);
-    return fba * dh + m.w * dg;
+    const T fba30 = m.eB0 - m.eB1 * c;             // 30 (f^beta - f^alpha)
+    const T u = e - e * e;                         // eta (1 - eta)
+    const T b = u * (T(1) - T(2) * e);
+    const T d = e * (s2 - e * e);
+    return fba30 * (u * u) + m.eW2 * b + m.eW4a * d;
 }
 
 }  // namespace pf
