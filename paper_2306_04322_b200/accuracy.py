@@ -25,8 +25,7 @@ import time
 import numpy as np
 
 
-def eq22_percent(phi, ref):
-    return 100.0 * float(np.sum((phi - ref) ** 2) / np.sum(ref ** 2))
+from .metrics import eq22_percent  # noqa: E402  (Eq. 22; one harness definition, checked against the oracle's in tests/)
 
 
 def advance(pf, n, p, dx, dt, t_span, c, eta, method="fs", k2_kind=0):
@@ -54,6 +53,9 @@ def main():
     ap.add_argument("--ref-dt", type=float, default=1e-4)
     ap.add_argument("--t-end", type=float, default=100.0)
     ap.add_argument("--fd-max-steps", type=float, default=5e6)
+    ap.add_argument("--pre", default="fs", choices=["fs", "fd"],
+                    help="pre-evolution t = 0 -> 1 on the reference grid: the FS step at --ref-dt (stand-in) or, as the paper "
+                         "describes it (PAPER.md:65), explicit FD at 0.75 x its stability limit on that grid (sensitivity run)")
     ap.add_argument("--out", default=None)
     a = ap.parse_args()
     p, length = 4, 200.0
@@ -62,8 +64,13 @@ def main():
     c0, eta0, dx0 = synth.init_b((nr, nr), p)
     assert abs(dx0[0] - length / nr) < 1e-12
     # stand-in for the paper's pre-evolution, then the reference run
-    c1, eta1, s, sec = advance(pf, nr, p, length / nr, a.ref_dt, 1.0, c0, eta0)
-    print(f"pre-evolution t=0..1 on {nr}^2, dt={a.ref_dt:g}: {s} FS steps in {sec:.1f} s", flush=True)
+    if a.pre == "fd":
+        k2r = 8.0 / (length / nr) ** 2
+        pre_dt = min(0.75 * 2.0 / (M * k2r * (2 * rho2 + kc * k2r)), 2e-3)
+    else:
+        pre_dt = a.ref_dt
+    c1, eta1, s, sec = advance(pf, nr, p, length / nr, pre_dt, 1.0, c0, eta0, a.pre)
+    print(f"pre-evolution t=0..1 on {nr}^2, dt={pre_dt:g}: {s} {a.pre.upper()} steps in {sec:.1f} s", flush=True)
     cr, er, s, sec = advance(pf, nr, p, length / nr, a.ref_dt, a.t_end - 1.0, c1, eta1)
     print(f"reference     t=1..{a.t_end:g} on {nr}^2, dt={a.ref_dt:g}: {s} FS steps in {sec:.1f} s "
           f"(finite: {bool(np.isfinite(cr).all())})", flush=True)
@@ -94,7 +101,7 @@ def main():
             print(f"{n:>6} {name:>14} {dt:>10.3e} {steps:>9d} {sec:>8.2f} {ec:>11} {ee:>11}", flush=True)
     if a.out:
         with open(a.out, "w") as fh:
-            json.dump({"ref_grid": nr, "ref_dt": a.ref_dt, "t_end": a.t_end, "runs": rows}, fh, indent=1)
+            json.dump({"ref_grid": nr, "ref_dt": a.ref_dt, "pre": a.pre, "pre_dt": pre_dt, "t_end": a.t_end, "runs": rows}, fh, indent=1)
 
 
 if __name__ == "__main__":

@@ -164,6 +164,8 @@ template <typename T> cudaError_t col2d_shape(int nfft, int M, Col2dShapeInfo *o
 template <typename T> cudaError_t launch_col2d(int nfft, const Col2dParams<T> &p, int grid, cudaStream_t s);
 template <typename T> cudaError_t launch_fd_fused2d(const FdParams<T> &p, cudaStream_t s);
 template <typename T> cudaError_t launch_fd_fused3d(const FdParams<T> &p, cudaStream_t s);
+// 3D, nx >= 64, at most four order parameters (fd3d_kernels.cu); cudaErrorNotSupported otherwise
+template <typename T> cudaError_t launch_fd3d_march(const FdParams<T> &p, cudaStream_t s);
 template <typename T> cudaError_t launch_energy(const EnergyParams<T> &p, cudaStream_t s);
 
 #if defined(__CUDACC__)

@@ -310,3 +310,16 @@ def test_eq22_closed_forms(oracle):
     assert np.isclose(oracle.error_eq22(np.full((4, 6), 1.1), np.ones((4, 6))), 0.01, rtol=1e-12)
     with pytest.raises(RuntimeError):
         oracle.error_eq22(np.ones(4), np.zeros(4))
+
+
+def test_harness_eq22_agrees_with_the_oracle(oracle):
+    # accuracy.py and crossover.py report Eq. 22 through ONE harness function (paper_2306_04322_b200/metrics.py); it has
+    # to be the quantity the oracle defines (and the closed forms above pin), including which argument normalises
+    from paper_2306_04322_b200 import metrics
+    rng = np.random.default_rng(22)
+    for shape in ((50,), (12, 9), (5, 6, 7)):
+        ref = 0.5 + 0.2 * rng.standard_normal(shape)
+        phi = ref + 0.03 * rng.standard_normal(shape)
+        assert np.isclose(metrics.eq22(phi, ref), oracle.error_eq22(phi, ref), rtol=1e-13)
+        assert np.isclose(metrics.eq22_percent(phi, ref), 100.0 * oracle.error_eq22(phi, ref), rtol=1e-13)
+        assert not np.isclose(metrics.eq22(phi, ref), oracle.error_eq22(ref, phi), rtol=1e-6)

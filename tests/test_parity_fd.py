@@ -82,3 +82,28 @@ def test_fd_fused_3d_planes(oracle, n, n_eta, steps):
     dt = min(0.75 * 2.0 / (5.0 * kt2 * (4.0 + 3.0 * kt2)), 2e-3)
     (gc, geta), (rc, reta) = run_both(oracle, n=n, n_eta=n_eta, init="B", steps=steps, dt=dt, method="fd")
     assert rel_linf([gc, geta], [rc, reta]) < 1e-12
+
+
+@pytest.mark.parametrize("n,n_eta,steps,precision", [
+    ((64, 16, 16), 0, 30, "f64"), ((64, 16, 32), 1, 30, "f64"), ((128, 64, 16), 2, 25, "f64"), ((64, 32, 64), 3, 20, "f64"),
+    ((256, 16, 64), 4, 10, "f64"), ((64, 64, 128), 2, 12, "f64"), ((64, 64, 64), 6, 10, "f64"),
+    ((128, 32, 64), 2, 40, "f32"), ((64, 16, 32), 4, 40, "f32")])
+def test_fd_3d_pair_marching_kernel(oracle, n, n_eta, steps, precision):
+    # fd3d_kernels.cu (nx >= 64, up to four order parameters: two points per thread, z neighbours in registers): every
+    # field count it serves, tiles that wrap in x and y (nx = 64: one tile per row; ny = 16: two tiles per column),
+    # several z chunks with rings that wrap in z, both precisions; six order parameters take the older kernel
+    c, eta, dx = make_init("B", n, n_eta)
+    kt2 = sum(4.0 / d ** 2 for d in dx)
+    dt = min(0.75 * 2.0 / (5.0 * kt2 * (4.0 + 3.0 * kt2)), 2e-3)
+    (gc, geta), (rc, reta) = run_both(oracle, n=n, n_eta=n_eta, init="B", steps=steps, dt=dt, method="fd", precision=precision)
+    assert rel_linf([gc, geta], [rc, reta]) < (1e-12 if precision == "f64" else 1e-5)
+
+
+def test_fd_3d_anisotropic_spacing_noise(oracle):
+    # seeded noise (every point differs from its neighbours) and three different spacings: a transposed stencil weight
+    # or a wrong neighbour in the pair code shows up at once
+    n, dx = (64, 32, 16), (1.0, 0.8, 1.25)
+    kt2 = sum(4.0 / d ** 2 for d in dx)
+    dt = 0.5 * 2.0 / (5.0 * kt2 * (4.0 + 3.0 * kt2))
+    (gc, geta), (rc, reta) = run_both(oracle, n=n, n_eta=2, init="A", steps=50, dt=dt, method="fd", dx=dx)
+    assert rel_linf([gc, geta], [rc, reta]) < 1e-12
