@@ -123,7 +123,9 @@ col2d_kernel(const Col2dParams<T> p)
         }
         const int item = s_items[ic];
         if (item < 0) break;
-        const int op = item & 15, slot = (item >> 4) & 15, ub = item >> 8;
+        // block index over all replicas of a batched context (pf_create_batch): gb = replica * nblk + block
+        const int op = item & 15, slot = (item >> 4) & 15, gb = item >> 8;
+        const int rep = gb / p.nblk, ub = gb - rep * p.nblk;
 
         // ---- the columns of this item ----
         int u = ub * TP + (sl >> 1);
@@ -134,8 +136,9 @@ col2d_kernel(const Col2dParams<T> p)
         const bool store_ok = valid && (side == 0 || zcolB != zcolA);
         const C wx = p.twx[u];                     // exp(-2 pi i u / nx)
         const T base2 = p.kx2[kx];
-        C *carry = p.carry + ((long)ub * E) * GT + tid;
-        C *zfield = p.zst + (long)slot * p.zfs;
+        C *carry = p.carry + ((long)gb * E) * GT + tid;
+        const long rep_off = (long)rep * N * M;            // rows of this replica within a field
+        C *zfield = p.zst + (long)slot * p.zfs + rep_off;
 
         // the carried spectrum was written a step ago: ask the L2 for this item's slice (first item) and the next item's
         if (ic == 0) prefetch_carry<T, E, GT>(p, item, tid);
@@ -144,7 +147,7 @@ col2d_kernel(const Col2dParams<T> p)
         C v[E];
         if (op != COL2D_C_INV) {
             // E = (za + conj zb)/2, O = -(i/2)(za - conj zb), U_u = E + W O (side 0), U_{M-u} = conj(E - W O) (side 1)
-            const C *src = (op == COL2D_C_FWD || op == COL2D_C_FULL) ? p.zg : zfield;
+            const C *src = (op == COL2D_C_FWD || op == COL2D_C_FULL) ? p.zg + rep_off : zfield;
 #pragma unroll
             for (int q = 0; q < E; ++q) {
                 const long i = j + q * TT;
@@ -182,15 +185,15 @@ col2d_kernel(const Col2dParams<T> p)
             }
             if (op == COL2D_C_FWD) {
                 __syncthreads();                               // the carry writes of the whole CTA precede the flag
-                if (tid == 0) { __threadfence(); st_release(p.flags + ub, 1); }
+                if (tid == 0) { __threadfence(); st_release(p.flags + gb, 1); }
                 continue;
             }
 #pragma unroll
             for (int q = 0; q < E; ++q) v[q] = cscale(v[q], sN);
         } else {   // COL2D_C_INV
             if (tid == 0) {
-                while (ld_acquire(p.flags + ub) == 0) __nanosleep(100);
-                p.flags[ub] = 0;                   // one producer and one consumer per launch
+                while (ld_acquire(p.flags + gb) == 0) __nanosleep(100);
+                p.flags[gb] = 0;                   // one producer and one consumer per launch
             }
             __syncthreads();
 #pragma unroll

@@ -56,6 +56,7 @@ __global__ void __launch_bounds__(256) fd_fused2d_kernel(const FdParams<T> p)
     T *smu = sc + CW * CH;
     T *se = smu + EW * EH;
     const int x0 = blockIdx.x * TX, y0 = blockIdx.y * TY;
+    const long rep = (long)blockIdx.z * p.N;             // replica of a batched context
     const int mx = p.nx - 1, my = p.ny - 1;
     constexpr int ne = NE;                 // compile-time field count: the per-field loops unroll into fixed offsets
 
@@ -66,12 +67,12 @@ __global__ void __launch_bounds__(256) fd_fused2d_kernel(const FdParams<T> p)
     grid_dependents_launch();
 
     for (int ly = ty; ly < CH; ly += TYS) {
-        const T *row = p.c + (long)((y0 + ly - 2) & my) * p.nx;
+        const T *row = p.c + rep + (long)((y0 + ly - 2) & my) * p.nx;
         cp_async_elem(sc + ly * CW + tx, row + ((x0 + tx - 2) & mx));
         if (tx < 4) cp_async_elem(sc + ly * CW + TX + tx, row + ((x0 + TX + tx - 2) & mx));
     }
     for (int k = 0; k < ne; ++k) {
-        const T *ek = p.eta + (long)k * p.N;
+        const T *ek = p.eta + (long)k * p.fs + rep;
         T *sk = se + k * (EW * EH);
         for (int ly = ty; ly < EH; ly += TYS) {
             const T *row = ek + (long)((y0 + ly - 1) & my) * p.nx;
@@ -101,7 +102,7 @@ __global__ void __launch_bounds__(256) fd_fused2d_kernel(const FdParams<T> p)
     // kernels (ii) + (iii) on the tile
     for (int ly = ty; ly < TY; ly += TYS) {
         const int lx = tx;
-        const long g = (long)(y0 + ly) * p.nx + (x0 + lx);
+        const long g = rep + (long)(y0 + ly) * p.nx + (x0 + lx);
         const int e0 = (ly + 1) * EW + (lx + 1);
         const T c = sc[(ly + 2) * CW + (lx + 2)];
         const T *mu = smu + e0;
@@ -112,7 +113,7 @@ __global__ void __launch_bounds__(256) fd_fused2d_kernel(const FdParams<T> p)
         for (int k = 0; k < ne; ++k) {
             const T *e = se + k * (EW * EH) + e0;
             const T le = p.rdx2[0] * (e[1] + e[-1] - T(2) * e[0]) + p.rdx2[1] * (e[EW] + e[-EW] - T(2) * e[0]);
-            p.eta_new[(long)k * p.N + g] = e[0] - p.m.dtL * (dfdeta(p.m, c, e[0], s2) - p.m.kappa_eta * le);
+            p.eta_new[(long)k * p.fs + g] = e[0] - p.m.dtL * (dfdeta(p.m, c, e[0], s2) - p.m.kappa_eta * le);
         }
     }
 }
@@ -276,7 +277,7 @@ template <typename T, int TX, int TY, int NE> static cudaError_t launch_fd_fused
     }
     // programmatic dependent launch: consecutive steps cannot overlap, but the launch latency of step t+1 hides
     // behind the tail of step t
-    return launch_pdl(kern, dim3((unsigned)(p.nx / TX), (unsigned)(p.ny / TY)), dim3(256), smem, s, true, p);
+    return launch_pdl(kern, dim3((unsigned)(p.nx / TX), (unsigned)(p.ny / TY), (unsigned)(p.nbatch > 0 ? p.nbatch : 1)), dim3(256), smem, s, true, p);
 }
 template <typename T, int TX, int TY> static cudaError_t launch_fd_fused2d_inst(const FdParams<T> &p, cudaStream_t s)
 {

@@ -38,7 +38,9 @@ const int kGraphSteps = 8;              // steps per captured graph (pf_step_fs 
 struct pf_ctx {
     pf_params p;
     int F = 1, M = 0, P2 = 0;
-    long N = 0;
+    long N = 0;                          // grid points of ONE replica
+    int B = 1;                           // replicas advanced together (pf_create_batch; 2D only)
+    int c2_nblk = 0;                     // column blocks per replica of the 2D last-axis kernel
     size_t w = 8;
     int device = 0;                      // the CUDA device the context was created on (every call checks it is current)
     cudaStream_t stream = nullptr;
@@ -170,8 +172,8 @@ template <typename T> RowParams<T> row_params(pf_ctx *c)
     RowParams<T> r;
     r.zst = (C *)c->zst; r.zg = (C *)c->zg; r.real = (T *)c->real[c->cur];
     r.tw = (const C *)c->tw_m;
-    r.zfs = c->N / 2; r.rfs = c->N;
-    r.nrows = c->p.n[1] * c->p.n[2]; r.F = c->F;
+    r.zfs = c->B * (c->N / 2); r.rfs = c->B * c->N;   // replicas are further rows of every field
+    r.nrows = c->p.n[1] * c->p.n[2] * c->B; r.F = c->F;
     r.carveout = c->carveout;
     r.m = make_model<T>(c->p);
 #ifdef PF_TRACE
@@ -204,7 +206,7 @@ template <typename T> Col2dParams<T> col2d_params(pf_ctx *c, bool init, bool pdl
     Col2dParams<T> q;
     memset(&q, 0, sizeof(q));
     q.zst = (C *)c->zst; q.zg = (const C *)c->zg; q.carry = (C *)c->carry;
-    q.zfs = c->N / 2; q.M = c->M;
+    q.zfs = c->B * (c->N / 2); q.M = c->M; q.nblk = c->c2_nblk;
     q.sched = init ? c->c2_sched_init : c->c2_sched;
     q.per_cta = init ? c->c2_per_init : c->c2_per;
     q.flags = c->c2_flags;
@@ -251,7 +253,7 @@ template <typename T> int fs_one_step(pf_ctx *c, cudaEvent_t *events, int only =
 {
     typedef typename V2<T>::type C;
     const int ny = c->p.n[1], nz = c->p.n[2];
-    const long zfs = c->N / 2;
+    const long zfs = c->B * (c->N / 2);
     const bool pdl = events == nullptr && only < 0;
     KernelTimer kt(c, events);
     auto want = [&](int k) { return only < 0 || only == k; };
@@ -398,12 +400,12 @@ template <typename T> int step_fd(pf_ctx *c, int nsteps)
     int rc = to_real<T>(c);
     if (rc) return rc;
     FdParams<T> f;
-    f.nx = c->p.n[0]; f.ny = c->p.n[1]; f.nz = c->p.n[2]; f.N = c->N;
+    f.nx = c->p.n[0]; f.ny = c->p.n[1]; f.nz = c->p.n[2]; f.N = c->N; f.fs = c->B * c->N; f.nbatch = c->B;
     for (int d = 0; d < 3; ++d) f.rdx2[d] = (d < c->p.ndim) ? (T)(1.0 / (c->p.dx[d] * c->p.dx[d])) : (T)0;
     f.m = make_model<T>(c->p);
     for (int s = 0; s < nsteps; ++s) {
         T *cu = (T *)c->real[c->cur], *nw = (T *)c->real[c->cur ^ 1];
-        f.c = cu; f.eta = cu + c->N; f.c_new = nw; f.eta_new = nw + c->N;
+        f.c = cu; f.eta = cu + c->B * c->N; f.c_new = nw; f.eta_new = nw + c->B * c->N;
         if (c->p.ndim == 2) {
             PF_CK(c, launch_fd_fused2d<T>(f, c->stream));
             c->launches += 1;
@@ -473,11 +475,26 @@ bool on_device(const pf_ctx *c)
     return cudaGetDevice(&d) == cudaSuccess && d == c->device;
 }
 
-int copy_fields(pf_ctx *c, void *dc, void *deta, const void *sc, const void *seta, cudaMemcpyKind kind)
+// Fields between the caller's arrays and real[]. Caller: c [B][N], eta [B][p][N] (replica-major); library: [F][B][N]
+// (a replica is a run of rows of every field). to_lib: caller -> library, else library -> caller.
+int copy_fields(pf_ctx *c, void *user_c, void *user_eta, void *lib, bool to_lib, cudaMemcpyKind kind)
 {
-    const size_t fb = (size_t)c->N * c->w;
-    PF_CK(c, cudaMemcpyAsync(dc, sc, fb, kind, c->stream));
-    if (c->p.n_eta > 0) PF_CK(c, cudaMemcpyAsync(deta, seta, fb * c->p.n_eta, kind, c->stream));
+    const size_t fb = (size_t)c->N * c->w;               // one field of one replica
+    char *lc = (char *)lib, *le = lc + fb * c->B;
+    const int p = c->p.n_eta;
+    if (to_lib) PF_CK(c, cudaMemcpyAsync(lc, user_c, fb * c->B, kind, c->stream));
+    else PF_CK(c, cudaMemcpyAsync(user_c, lc, fb * c->B, kind, c->stream));
+    if (p == 0) return PF_OK;
+    if (c->B == 1) {
+        if (to_lib) PF_CK(c, cudaMemcpyAsync(le, user_eta, fb * p, kind, c->stream));
+        else PF_CK(c, cudaMemcpyAsync(user_eta, le, fb * p, kind, c->stream));
+        return PF_OK;
+    }
+    for (int f = 0; f < p; ++f) {                        // B runs of N elements: pitch p*N on the caller's side, N on ours
+        char *ue = (char *)user_eta + fb * f, *lf = le + fb * c->B * f;
+        if (to_lib) PF_CK(c, cudaMemcpy2DAsync(lf, fb, ue, fb * p, fb, c->B, kind, c->stream));
+        else PF_CK(c, cudaMemcpy2DAsync(ue, fb * p, lf, fb, fb, c->B, kind, c->stream));
+    }
     return PF_OK;
 }
 
@@ -528,9 +545,11 @@ void pf_destroy(pf_ctx *c)
     delete c;
 }
 
-int pf_create(const pf_params *p, pf_ctx **out)
+static int create_impl(const pf_params *p, int nbatch, pf_ctx **out)
 {
     if (!p || !out) return PF_EINVAL;
+    if (nbatch < 1 || nbatch > 4096) return PF_EINVAL;
+    if (nbatch > 1 && p->ndim != 2) return PF_EUNSUPPORTED;
     if (p->ndim != 2 && p->ndim != 3) return PF_EINVAL;
     if (p->n_eta < 0 || p->n_eta > 8) return PF_EINVAL;
     if (!(p->dt > 0.0)) return PF_EINVAL;
@@ -547,9 +566,10 @@ int pf_create(const pf_params *p, pf_ctx **out)
     pf_ctx *c = new (std::nothrow) pf_ctx();
     if (!c) return PF_ENOMEM;
     c->p = *p;
+    c->B = nbatch;
     c->device = dev;
-    { const char *e = getenv("PF_WCOL"); c->use_wcol = (e && e[0] == '1'); }
-    { const char *e = getenv("PF_COL2D_LEGACY"); c->legacy_col2d = (e && e[0] == '1'); }
+    { const char *e = getenv("PF_WCOL"); c->use_wcol = (e && e[0] == '1' && nbatch == 1); }
+    { const char *e = getenv("PF_COL2D_LEGACY"); c->legacy_col2d = (e && e[0] == '1' && nbatch == 1); }
     { const char *e = getenv("PF_FD3D_LEGACY"); c->legacy_fd3d = (e && e[0] == '1'); }
     { const char *e = getenv("PF_NO_GRAPH"); if (e && e[0] == '1') c->graph_ok = false; }
     if (p->ndim == 2) { c->p.n[2] = 1; c->p.dx[2] = 1.0; }
@@ -572,12 +592,12 @@ int pf_create(const pf_params *p, pf_ctx **out)
         e = cudaMemset(*dst, 0, bytes);
         return e == cudaSuccess ? PF_OK : PF_ECUDA;
     };
-    const size_t fb = (size_t)c->N * c->w;                 // one real field
+    const size_t fb = (size_t)c->N * c->w * c->B;          // one real field of every replica
     int rc;
     if ((rc = alloc(&c->real[0], fb * c->F)) || (rc = alloc(&c->real[1], fb * c->F)) ||
         (rc = alloc(&c->zst, fb * c->F)) || (rc = alloc(&c->zg, fb)) ||
         (rc = alloc((void **)&c->acc, sizeof(double) * 32)) || (rc = alloc((void **)&c->queue, sizeof(int) * 4)) ||
-        (rc = alloc(&c->park, (size_t)(c->P2 + 16) * c->p.n[1] * c->p.n[2] * 2 * c->w)))
+        (rc = alloc(&c->park, (size_t)(c->P2 + 16) * c->p.n[1] * c->p.n[2] * 2 * c->w * c->B)))
         return fail(rc);
     if (p->ndim == 3) {
         const size_t pb = (size_t)c->p.n[2] * c->p.n[1] * c->P2 * 2 * c->w;
@@ -590,13 +610,15 @@ int pf_create(const pf_params *p, pf_ctx **out)
         cudaError_t e = (p->precision == PF_F64) ? col2d_shape<double>(c->p.n[1], c->M, &si) : col2d_shape<float>(c->p.n[1], c->M, &si);
         if (e != cudaSuccess) { c->cuda_err = cudaGetErrorString(e); cudaGetLastError(); return fail(PF_ECUDA); }
         c->carveout = si.carveout_pct;
+        c->c2_nblk = si.nblk;
+        const int nblk_all = si.nblk * c->B;               // the replicas' column blocks are dealt out together
         std::vector<int> sched, sched_init;
-        col2d_schedule(si.nblk, p->n_eta, si.slots, &c->c2_grid, &c->c2_per, sched);
-        col2d_schedule_init(si.nblk, si.slots, &c->c2_grid_init, &c->c2_per_init, sched_init);
-        if ((rc = alloc(&c->carry, (size_t)si.carry_elems * 2 * c->w)) ||
+        col2d_schedule(nblk_all, p->n_eta, si.slots, &c->c2_grid, &c->c2_per, sched);
+        col2d_schedule_init(nblk_all, si.slots, &c->c2_grid_init, &c->c2_per_init, sched_init);
+        if ((rc = alloc(&c->carry, (size_t)si.carry_elems * c->B * 2 * c->w)) ||
             (rc = alloc((void **)&c->c2_sched, sizeof(int) * sched.size())) ||
             (rc = alloc((void **)&c->c2_sched_init, sizeof(int) * sched_init.size())) ||
-            (rc = alloc((void **)&c->c2_flags, sizeof(int) * (size_t)si.nblk)))
+            (rc = alloc((void **)&c->c2_flags, sizeof(int) * (size_t)nblk_all)))
             return fail(rc);
         if (cudaMemcpy(c->c2_sched, sched.data(), sizeof(int) * sched.size(), cudaMemcpyHostToDevice) != cudaSuccess ||
             cudaMemcpy(c->c2_sched_init, sched_init.data(), sizeof(int) * sched_init.size(), cudaMemcpyHostToDevice) != cudaSuccess) {
@@ -616,13 +638,16 @@ int pf_create(const pf_params *p, pf_ctx **out)
     return PF_OK;
 }
 
+int pf_create(const pf_params *p, pf_ctx **out) { return create_impl(p, 1, out); }
+int pf_create_batch(const pf_params *p, int nbatch, pf_ctx **out) { return create_impl(p, nbatch, out); }
+int pf_batch_size(const pf_ctx *c) { return c ? c->B : 0; }
+
 int pf_set_fields(pf_ctx *c, const void *fc, const void *eta, int where)
 {
     if (!c || !fc || (c->p.n_eta > 0 && !eta)) return PF_EINVAL;
     if (where != PF_HOST && where != PF_DEVICE) return PF_EINVAL;
     if (!on_device(c)) return PF_EINVAL;
-    char *dst = (char *)c->real[c->cur];
-    int rc = copy_fields(c, dst, dst + (size_t)c->N * c->w, fc, eta,
+    int rc = copy_fields(c, const_cast<void *>(fc), const_cast<void *>(eta), c->real[c->cur], true,
                          where == PF_HOST ? cudaMemcpyHostToDevice : cudaMemcpyDeviceToDevice);
     if (rc) return rc;
     if (where == PF_HOST) PF_CK(c, cudaStreamSynchronize(c->stream));
@@ -640,8 +665,7 @@ int pf_get_fields(pf_ctx *c, void *fc, void *eta, int where)
     if (c->state == ST_NONE || c->state == ST_TIMING) return PF_ESTATE;
     int rc = (c->p.precision == PF_F64) ? to_real<double>(c) : to_real<float>(c);
     if (rc) return rc;
-    const char *src = (const char *)c->real[c->cur];
-    rc = copy_fields(c, fc, eta, src, src + (size_t)c->N * c->w,
+    rc = copy_fields(c, fc, eta, c->real[c->cur], false,
                      where == PF_HOST ? cudaMemcpyDeviceToHost : cudaMemcpyDeviceToDevice);
     if (rc) return rc;
     if (where == PF_HOST) PF_CK(c, cudaStreamSynchronize(c->stream));
@@ -670,6 +694,7 @@ int pf_free_energy(pf_ctx *c, int gradient_kind, double *out)
 {
     if (!c || !out || (gradient_kind != 0 && gradient_kind != 1)) return PF_EINVAL;
     if (!on_device(c)) return PF_EINVAL;
+    if (c->B > 1) return PF_EUNSUPPORTED;              /* one replica at a time: read the fields out */
     if (c->state == ST_NONE || c->state == ST_TIMING) return PF_ESTATE;
     return (c->p.precision == PF_F64) ? free_energy<double>(c, gradient_kind, out)
                                       : free_energy<float>(c, gradient_kind, out);

@@ -115,14 +115,15 @@ enum Col2dOp {
 };
 template <typename T> struct Col2dParams {
     typedef typename V2<T>::type C;
-    C       *zst;            // [F][ny][M] z-form state; slot s at zst + s*zfs (slot 0 = c, written by C_INV / C_FULL)
-    const C *zg;             // [ny][M] z-form of g = df/dc
-    C       *carry;          // c^ in the kernel's thread-linear order: [nblk][E][THREADS]
+    C       *zst;            // [F][B][ny][M] z-form state of B replicas; slot s at zst + s*zfs (slot 0 = c, written by C_INV / C_FULL)
+    const C *zg;             // [B][ny][M] z-form of g = df/dc
+    C       *carry;          // c^ in the kernel's thread-linear order: [B*nblk][E][THREADS]
     long     zfs;
     int      M;              // nx/2 = pitch of the z-form rows
+    int      nblk;           // column blocks per replica (items carry replica * nblk + block)
     int      per_cta;        // items per CTA in sched (padded with -1; at most Col2dShapeInfo::max_items)
     const int *sched;        // [grid][per_cta] items: op | slot << 4 | block << 8
-    int     *flags;          // [nblk] C_FWD -> C_INV hand-off, zero between launches
+    int     *flags;          // [B*nblk] C_FWD -> C_INV hand-off, zero between launches
     int      pdl;
     const C *tw;             // exp(-2 pi i k / ny)
     const C *twx;            // exp(-2 pi i k / nx), k <= M/2
@@ -141,6 +142,8 @@ template <typename T> struct FdParams {
     T       *c_new, *eta_new;
     int      nx, ny, nz;
     long     N;              // nx*ny*nz
+    long     fs;             // stride between the eta fields (N x replicas of a batched 2D context; replica b at + b*N)
+    int      nbatch;         // replicas (2D only: blockIdx.z)
     T        rdx2[3];        // 1/dx^2 per axis (rdx2[2] = 0 in 2D)
     Model<T> m;
 };

@@ -19,7 +19,7 @@ PF_F32, PF_F64 = 0, 1
 PF_HOST, PF_DEVICE = 0, 1
 PF_OK, PF_EINVAL, PF_ENOMEM, PF_ECUDA, PF_ESTATE, PF_EUNSUPPORTED = 0, -1, -2, -3, -4, -5
 
-EXPORTS = ["pf_create", "pf_set_fields", "pf_step_fs", "pf_step_fd", "pf_get_fields", "pf_free_energy",
+EXPORTS = ["pf_create", "pf_create_batch", "pf_batch_size", "pf_set_fields", "pf_step_fs", "pf_step_fd", "pf_get_fields", "pf_free_energy",
            "pf_set_dt", "pf_launch_count", "pf_set_profiling", "pf_num_fs_kernels", "pf_fs_kernel_ms", "pf_launch_fs_kernel",
            "pf_fs_kernel_name", "pf_strerror", "pf_last_cuda_error", "pf_destroy"]
 
@@ -56,6 +56,10 @@ def lib() -> ctypes.CDLL:
         vp, pp = ctypes.c_void_p, ctypes.POINTER(PfParams)
         L.pf_create.restype = ctypes.c_int
         L.pf_create.argtypes = [pp, ctypes.POINTER(vp)]
+        L.pf_create_batch.restype = ctypes.c_int
+        L.pf_create_batch.argtypes = [pp, ctypes.c_int, ctypes.POINTER(vp)]
+        L.pf_batch_size.restype = ctypes.c_int
+        L.pf_batch_size.argtypes = [vp]
         L.pf_set_fields.restype = ctypes.c_int
         L.pf_set_fields.argtypes = [vp, vp, vp, ctypes.c_int]
         L.pf_get_fields.restype = ctypes.c_int
@@ -111,19 +115,26 @@ def make_params(n, n_eta=4, dx=1.0, dt=5e-3, M=5.0, L=5.0, kappa_c=3.0, kappa_et
 
 
 class Context:
-    """Thin RAII wrapper of pf_ctx. Host arrays are numpy, device arrays anything with `data_ptr()` (torch)."""
+    """Thin RAII wrapper of pf_ctx. Host arrays are numpy, device arrays anything with `data_ptr()` (torch).
+    nbatch = B > 0: pf_create_batch, B independent replicas per launch; fields are then c [B, ny, nx], eta [B, p, ny, nx]."""
 
-    def __init__(self, n, **kw):
+    def __init__(self, n, nbatch=None, **kw):
         self.params = make_params(n, **kw)
         self.n = tuple(int(v) for v in n)
         self.n_eta = self.params.n_eta
         self.dtype = np.float64 if self.params.precision == PF_F64 else np.float32
+        self.nbatch = None if nbatch is None else int(nbatch)
         self.shape = tuple(reversed(self.n))
+        self._cshape = self.shape if nbatch is None else (self.nbatch,) + self.shape
+        self._eshape = (self.n_eta,) + self.shape if nbatch is None else (self.nbatch, self.n_eta) + self.shape
         self._h = ctypes.c_void_p()
-        rc = lib().pf_create(ctypes.byref(self.params), ctypes.byref(self._h))
+        if nbatch is None:
+            rc, what = lib().pf_create(ctypes.byref(self.params), ctypes.byref(self._h)), "pf_create"
+        else:
+            rc, what = lib().pf_create_batch(ctypes.byref(self.params), self.nbatch, ctypes.byref(self._h)), "pf_create_batch"
         if rc != PF_OK:
             self._h = ctypes.c_void_p()
-            raise PfError(rc, "pf_create", lib().pf_strerror(rc).decode())
+            raise PfError(rc, what, lib().pf_strerror(rc).decode())
 
     def _ck(self, rc, what):
         if rc != PF_OK:
@@ -134,13 +145,13 @@ class Context:
 
     # ---- host (numpy) ----
     def set_fields(self, c, eta):
-        c = np.ascontiguousarray(c, dtype=self.dtype).reshape(self.shape)
-        eta = np.ascontiguousarray(eta, dtype=self.dtype).reshape((self.n_eta,) + self.shape)
+        c = np.ascontiguousarray(c, dtype=self.dtype).reshape(self._cshape)
+        eta = np.ascontiguousarray(eta, dtype=self.dtype).reshape(self._eshape)
         self._ck(lib().pf_set_fields(self._h, c.ctypes.data, eta.ctypes.data if self.n_eta else None, PF_HOST), "pf_set_fields")
 
     def get_fields(self):
-        c = np.empty(self.shape, dtype=self.dtype)
-        eta = np.empty((self.n_eta,) + self.shape, dtype=self.dtype)
+        c = np.empty(self._cshape, dtype=self.dtype)
+        eta = np.empty(self._eshape, dtype=self.dtype)
         self._ck(lib().pf_get_fields(self._h, c.ctypes.data, eta.ctypes.data if self.n_eta else None, PF_HOST), "pf_get_fields")
         return c, eta
 
