@@ -63,6 +63,7 @@ struct pf_ctx {
     bool carry_valid = false;
     int *c2_sched = nullptr, *c2_sched_init = nullptr, *c2_flags = nullptr;
     int c2_grid = 0, c2_per = 0, c2_grid_init = 0, c2_per_init = 0;
+    int sg_cs = 0;                       // > 0: cluster size of the resident small-grid kernel (sgrid_kernels.cu) serving this context
     int carveout = 0;                    // shared-memory carve-out both kernels of a 2D step run with (percent; 0: unset)
     TraceBuf *trace = nullptr;           // -DPF_TRACE builds only
     long long launches = 0;
@@ -307,14 +308,14 @@ template <typename T> int fs_one_step(pf_ctx *c, cudaEvent_t *events, int only =
 }
 
 // real fields -> z-form state (and, in 3D, the carried (kx,ky)-spectral planes of c)
-template <typename T> int to_spectral(pf_ctx *c)
+template <typename T> int to_spectral(pf_ctx *c, bool need_carry = true)
 {
     if (c->state == ST_REAL) {
         RowParams<T> r = row_params<T>(c);
         PF_CK(c, launch_row<T>(ROW_SET, c->p.n[0], r, c->stream)); ++c->launches;
         c->state = ST_BOTH;
     }
-    if (c->p.ndim == 2 && c->carry && !c->carry_valid) {
+    if (c->p.ndim == 2 && c->carry && !c->carry_valid && need_carry) {
         PF_CK(c, launch_col2d<T>(c->p.n[1], col2d_params<T>(c, true, false), c->c2_grid_init, c->stream)); ++c->launches;
         c->carry_valid = true;
     }
@@ -337,6 +338,21 @@ template <typename T> int to_real(pf_ctx *c)
 
 template <typename T> int step_fs(pf_ctx *c, int nsteps)
 {
+    if (c->sg_cs > 0 && !c->profiling) {
+        // small square 2D grids: every step of the call inside ONE launch, state resident in a cluster's shared memory
+        typedef typename V2<T>::type C;
+        int rc = to_spectral<T>(c, false);
+        if (rc) return rc;
+        SgParams<T> q;
+        q.zst = (C *)c->zst; q.zfs = c->B * (c->N / 2); q.F = c->F; q.nsteps = nsteps;
+        q.tw_m = (const C *)c->tw_m; q.tw_y = (const C *)c->tw_y; q.twx = (const C *)c->tw_nx;
+        q.kx2 = (const T *)c->kx2; q.ky2 = (const T *)c->ky2;
+        q.m = make_model<T>(c->p);
+        PF_CK(c, launch_sgrid<T>(c->p.n[0], c->p.n[1], q, c->sg_cs, c->B, c->stream)); ++c->launches;
+        c->carry_valid = false;          // the kernel re-transforms c every step; the carried spectrum is stale now
+        c->state = ST_SPECTRAL;
+        return PF_OK;
+    }
     int rc = to_spectral<T>(c);
     if (rc) return rc;
     if (c->profiling) {
@@ -624,6 +640,26 @@ static int create_impl(const pf_params *p, int nbatch, pf_ctx **out)
             cudaMemcpy(c->c2_sched_init, sched_init.data(), sizeof(int) * sched_init.size(), cudaMemcpyHostToDevice) != cudaSuccess) {
             cudaGetLastError();
             return fail(PF_ECUDA);
+        }
+    }
+    if (p->ndim == 2) {
+        // Square grids up to 64^2 run pf_step_fs in the cluster-resident kernel (sgrid_kernels.cu): 64^2, c + 2 eta, fp64:
+        // 4.7 us per step against 11.0 us on the two-kernel path; at 128^2 the two paths are level and the two-kernel path
+        // stays (profiles/r2_small_grids.md). A single simulation takes a cluster of 16 CTAs, a batch as many CTAs per
+        // replica as keep the whole batch on the machine at once.
+        // PF_RESIDENT=0: two-kernel path for every size (A/B runs); PF_SG_CLUSTER=<n>: resident path with clusters of >= n
+        // CTAs for every size that sgrid_kernels.cu serves and that fits.
+        const char *er = getenv("PF_RESIDENT"), *ec = getenv("PF_SG_CLUSTER");
+        if (!(er && er[0] == '0') && (ec || (p->n[0] == p->n[1] && p->n[0] <= 64))) {
+            int sms = 148;
+            cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+            int want = ec ? atoi(ec) : (c->B > 1 ? sms / c->B : 16);
+            if (want < 1) want = 1;
+            if (want > 16) want = 16;
+            while (want & (want - 1)) want &= want - 1;
+            c->sg_cs = (p->precision == PF_F64) ? sgrid_plan<double>(p->n[0], p->n[1], c->F, want)
+                                                : sgrid_plan<float>(p->n[0], p->n[1], c->F, want);
+            cudaGetLastError();
         }
     }
 #ifdef PF_TRACE

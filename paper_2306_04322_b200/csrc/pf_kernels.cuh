@@ -136,6 +136,19 @@ template <typename T> struct Col2dParams {
 // predecessor's last CTAs only if both run with the SAME carve-out: the x kernel is given this value too.
 struct Col2dShapeInfo { int tp, e, threads, max_items, nblk, slots, carveout_pct; long carry_elems; };
 
+// small 2D grids resident in the shared memory of a thread-block cluster (sgrid_kernels.cu)
+template <typename T> struct SgParams {
+    typedef typename V2<T>::type C;
+    C       *zst;            // [F][B][ny][M] z-form state in global memory: read at the start, written at the end
+    long     zfs;            // field stride (= B*ny*M)
+    int      F;              // 1 + n_eta
+    int      nsteps;         // steps of Algorithm 1 to run inside the launch
+    const C *tw_m, *tw_y;    // exp(-2 pi i k / M), exp(-2 pi i k / ny)
+    const C *twx;            // exp(-2 pi i k / nx), k <= M/2
+    const T *kx2, *ky2;      // |xi_x|^2 (M+1 entries), |xi_y|^2
+    Model<T> m;
+};
+
 // FD path
 template <typename T> struct FdParams {
     const T *c, *eta;        // time-t fields
@@ -165,6 +178,8 @@ template <typename T> cudaError_t launch_col(int mode, int nfft, int nslots, int
 template <typename T> cudaError_t launch_wcol2d(int nfft, int nslots, const ColParams<T> &p, cudaStream_t s);
 template <typename T> cudaError_t col2d_shape(int nfft, int M, Col2dShapeInfo *o);
 template <typename T> cudaError_t launch_col2d(int nfft, const Col2dParams<T> &p, int grid, cudaStream_t s);
+template <typename T> int sgrid_plan(int nx, int ny, int F, int want);
+template <typename T> cudaError_t launch_sgrid(int nx, int ny, const SgParams<T> &p, int cs, int nbatch, cudaStream_t s);
 template <typename T> cudaError_t launch_fd_fused2d(const FdParams<T> &p, cudaStream_t s);
 template <typename T> cudaError_t launch_fd_fused3d(const FdParams<T> &p, cudaStream_t s);
 // 3D, nx >= 64, at most four order parameters (fd3d_kernels.cu); cudaErrorNotSupported otherwise
