@@ -401,6 +401,11 @@ def measure_workload(wl, K, W, env, full=True):
         kms[name] = stats(ts)["median"] / (rounds * len(ctxs))
     reset_fields(ctxs, reps)
     ksurvey, kdesign = bytes_model(n, p, w)
+    if "cluster_resident_step" in names:
+        # grids served by the cluster-resident kernel (sgrid_kernels.cu): one kernel runs the whole step; a launch of one
+        # step reads and writes the state once
+        ksurvey = {"cluster_resident_step": sum(ksurvey.values())}
+        kdesign = {"cluster_resident_step": 2 * F * R}
     survey_bytes, design_bytes = sum(ksurvey.values()), sum(kdesign.values())
     peak, peak_src = peaks()
     dom = max(kms, key=kms.get)
@@ -551,6 +556,71 @@ def measure_workload(wl, K, W, env, full=True):
     return line
 
 
+def small_grid_measurements(env):
+    """SURVEY 8(f)-4 (the paper's small-grid remark): configs[0]'s grid (64^2, c + 2 eta, fp64, seeded noise,
+    dt = 0.05) as ONE simulation -- cluster-resident kernel (default up to 64^2: pf_step_fs(K) is one launch) against the
+    two-kernel path (PF_RESIDENT=0 at pf_create) -- and as a batch of 64 replicas in one context (pf_create_batch)
+    against a loop over 64 contexts."""
+    torch, pf, stream = env["torch"], env["pf"], env["stream"]
+    from paper_2306_04322_b200 import synth
+    n, p, K = (64, 64), 2, 2000
+
+    def timed(fn):
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        torch.cuda.synchronize()
+        e0.record(stream)
+        fn()
+        e1.record(stream)
+        torch.cuda.synchronize()
+        return e0.elapsed_time(e1)
+
+    def single(resident, n=n, p=p):
+        old = os.environ.get("PF_RESIDENT")
+        if not resident:
+            os.environ["PF_RESIDENT"] = "0"
+        try:
+            c, eta = synth.init_a(n, p, seed=1)
+            with pf.Context(n, n_eta=p, dx=1.0, dt=0.05, stream=stream.cuda_stream) as cx:
+                cx.set_fields(c, eta)
+                cx.step_fs(50)
+                l0 = cx.launch_count()
+                ms = stats([timed(lambda: cx.step_fs(K)) for _ in range(5)])["median"]
+                launches = (cx.launch_count() - l0) // 5
+        finally:
+            if old is None:
+                os.environ.pop("PF_RESIDENT", None)
+            else:
+                os.environ["PF_RESIDENT"] = old
+        return {"value": 1e3 * K / ms, "unit": "steps/s", "us_per_step": 1e3 * ms / K, "launches_per_call_of_%d_steps" % K: int(launches)}
+
+    out = {"workload": "2D 64x64, c + 2 eta, fp64, seeded noise, dt = 0.05 (configs[0])",
+           "single_simulation_cluster_resident": single(True), "single_simulation_two_kernel_path": single(False),
+           "single_256sq_c_4eta_two_kernel_path": single(True, (256, 256), 4)}
+    B = 64
+    inits = [synth.init_a(n, p, seed=100 + b) for b in range(B)]
+    c0, e0 = np.stack([c for c, _ in inits]), np.stack([e for _, e in inits])
+    with pf.Context(n, n_eta=p, dx=1.0, dt=0.05, nbatch=B, stream=stream.cuda_stream) as cx:
+        cx.set_fields(c0, e0)
+        cx.step_fs(20)
+        msb = stats([timed(lambda: cx.step_fs(K // 4)) for _ in range(5)])["median"] / (K // 4)
+    cxs = [pf.Context(n, n_eta=p, dx=1.0, dt=0.05, stream=stream.cuda_stream) for _ in range(B)]
+    for b, cx in enumerate(cxs):
+        cx.set_fields(c0[b], e0[b])
+        cx.step_fs(4)
+
+    def loop():
+        for _ in range(20):
+            for cx in cxs:
+                cx.step_fs(1)
+    msl = stats([timed(loop) for _ in range(3)])["median"] / 20
+    for cx in cxs:
+        cx.close()
+    out["batch_of_64_replicas"] = {"one_context_replica_steps_per_s": 1e3 * B / msb, "us_per_step_of_all_replicas": 1e3 * msb,
+                                   "loop_over_64_contexts_replica_steps_per_s": 1e3 * B / msl, "ratio": msl / msb,
+                                   "note": "pf_create_batch(nbatch=64) + pf_step_fs(K) against pf_step_fs(1) on 64 contexts in turn"}
+    return out
+
+
 def spawn_ranks(args, argv):
     """python bench.py --gpus N outside torchrun: re-execute under torch.distributed.run with N ranks on this node."""
     port = 29500 + (os.getpid() % 2000)
@@ -582,6 +652,8 @@ def run_ours(args):
     line = measure_workload(args.workload, K, args.warmup, env, full=True)
     line["library"] = {"path": pf.SO_PATH, "override": bool(os.environ.get("PF_LIBPF")), "kernel_source_hash": kernel_source_hash()}
 
+    if rank == 0 and world == 1 and args.workload == "1024sq" and not args.no_small_grids:
+        line["small_grids"] = small_grid_measurements(env)
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
         allc = oracle_timing(args.workload, 8.0)
         one = oracle_timing(args.workload, 4.0, threads=1)
@@ -616,6 +688,7 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-cufft", action="store_true", help="skip the cuFFT side reference")
+    ap.add_argument("--no-small-grids", action="store_true", help="skip the 64^2 single-simulation / batch measurements")
     ap.add_argument("--allow-lib-override", action="store_true", help="accept PF_LIBPF (ablation builds; never for a reported number)")
     args = ap.parse_args()
     if args.also is None:

@@ -336,23 +336,26 @@ template <typename T> int to_real(pf_ctx *c)
     return PF_OK;
 }
 
+// small square 2D grids: every step of the call inside ONE launch, state resident in a cluster's shared memory
+template <typename T> int resident_steps(pf_ctx *c, int nsteps)
+{
+    typedef typename V2<T>::type C;
+    int rc = to_spectral<T>(c, false);
+    if (rc) return rc;
+    SgParams<T> q;
+    q.zst = (C *)c->zst; q.zfs = c->B * (c->N / 2); q.F = c->F; q.nsteps = nsteps;
+    q.tw_m = (const C *)c->tw_m; q.tw_y = (const C *)c->tw_y; q.twx = (const C *)c->tw_nx;
+    q.kx2 = (const T *)c->kx2; q.ky2 = (const T *)c->ky2;
+    q.m = make_model<T>(c->p);
+    PF_CK(c, launch_sgrid<T>(c->p.n[0], c->p.n[1], q, c->sg_cs, c->B, c->stream)); ++c->launches;
+    c->carry_valid = false;              // the kernel keeps its own copy of c^; the carried spectrum in global memory is stale now
+    c->state = ST_SPECTRAL;
+    return PF_OK;
+}
+
 template <typename T> int step_fs(pf_ctx *c, int nsteps)
 {
-    if (c->sg_cs > 0 && !c->profiling) {
-        // small square 2D grids: every step of the call inside ONE launch, state resident in a cluster's shared memory
-        typedef typename V2<T>::type C;
-        int rc = to_spectral<T>(c, false);
-        if (rc) return rc;
-        SgParams<T> q;
-        q.zst = (C *)c->zst; q.zfs = c->B * (c->N / 2); q.F = c->F; q.nsteps = nsteps;
-        q.tw_m = (const C *)c->tw_m; q.tw_y = (const C *)c->tw_y; q.twx = (const C *)c->tw_nx;
-        q.kx2 = (const T *)c->kx2; q.ky2 = (const T *)c->ky2;
-        q.m = make_model<T>(c->p);
-        PF_CK(c, launch_sgrid<T>(c->p.n[0], c->p.n[1], q, c->sg_cs, c->B, c->stream)); ++c->launches;
-        c->carry_valid = false;          // the kernel re-transforms c every step; the carried spectrum is stale now
-        c->state = ST_SPECTRAL;
-        return PF_OK;
-    }
+    if (c->sg_cs > 0 && !c->profiling) return resident_steps<T>(c, nsteps);
     int rc = to_spectral<T>(c);
     if (rc) return rc;
     if (c->profiling) {
@@ -758,6 +761,11 @@ int pf_launch_fs_kernel(pf_ctx *c, int which)
     if (!c || which < 0 || which >= pf_num_fs_kernels(c)) return PF_EINVAL;
     if (!on_device(c)) return PF_EINVAL;
     if (c->state == ST_NONE) return PF_ESTATE;   /* ST_TIMING is fine here */
+    if (c->sg_cs > 0) {                          /* the one kernel of a resident context: a launch of one step */
+        int r = (c->p.precision == PF_F64) ? resident_steps<double>(c, 1) : resident_steps<float>(c, 1);
+        c->state = ST_TIMING;
+        return r;
+    }
     int rc = (c->p.precision == PF_F64) ? to_spectral<double>(c) : to_spectral<float>(c);
     if (rc) return rc;
     rc = (c->p.precision == PF_F64) ? fs_one_step<double>(c, nullptr, which) : fs_one_step<float>(c, nullptr, which);
@@ -770,6 +778,7 @@ int pf_launch_fs_kernel(pf_ctx *c, int which)
 int pf_num_fs_kernels(const pf_ctx *c)
 {
     if (!c) return 0;
+    if (c->sg_cs > 0) return 1;
     return c->p.ndim == 2 ? 2 : 4;
 }
 double pf_fs_kernel_ms(pf_ctx *c, int which) { return (c && which >= 0 && which < c->nk) ? c->kms[which] : -1.0; }
@@ -778,6 +787,7 @@ const char *pf_fs_kernel_name(const pf_ctx *c, int which)
     static const char *k2d[] = {"row_c2r_nonlinear_r2c", "col_y_fft_update_ifft"};
     static const char *k3d[] = {"row_c2r_nonlinear_r2c", "col_y_fwd", "col_z_fft_update_ifft", "col_y_inv"};
     if (!c || which < 0 || which >= pf_num_fs_kernels(c)) return "";
+    if (c->sg_cs > 0) return "cluster_resident_step";
     return c->p.ndim == 2 ? k2d[which] : k3d[which];
 }
 
