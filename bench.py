@@ -650,6 +650,10 @@ def run_ours(args):
 
     K = args.steps if args.steps is not None else DEFAULT_STEPS[args.workload]
     line = measure_workload(args.workload, K, args.warmup, env, full=True)
+    if rank == 0:
+        line["fp64_fma_peak_tflops"] = {"measured": pf.fp64_fma_peak(),
+                                        "nominal_from_unit_counts": 148 * 64 * 2 * 1.965e9 / 1e12,
+                                        "how": "pf_fp64_fma_peak: independent DFMA chains, 4 x 1024 threads per SM, best of 3 launches"}
     line["library"] = {"path": pf.SO_PATH, "override": bool(os.environ.get("PF_LIBPF")), "kernel_source_hash": kernel_source_hash()}
 
     if rank == 0 and world == 1 and args.workload == "1024sq" and not args.no_small_grids:

@@ -124,6 +124,10 @@ long long pf_launch_count(const pf_ctx *ctx);
  * programmatic dependent launch; the trajectory is the same. A single bracketed launch carries a few microseconds
  * of event overhead: for per-kernel figures without it use pf_launch_fs_kernel. */
 int    pf_set_profiling(pf_ctx *ctx, int on);
+/* Measured fp64 FMA rate of the current device in TFLOP/s (2 flops per FMA): a 20-line kernel of independent DFMA chains,
+ * best of three timed launches. Diagnostic for the roofline notes (the Fourier-spectral kernels are
+ * bound by fp64 issue and shared memory as much as by HBM). Synchronises the device. PF_EINVAL / PF_ECUDA on failure. */
+int    pf_fp64_fma_peak(double *tflops);
 int    pf_num_fs_kernels(const pf_ctx *ctx);
 double pf_fs_kernel_ms(pf_ctx *ctx, int which);
 const char *pf_fs_kernel_name(const pf_ctx *ctx, int which);

@@ -519,6 +519,22 @@ int copy_fields(pf_ctx *c, void *user_c, void *user_eta, void *lib, bool to_lib,
 
 }  // namespace
 
+// fp64 FMA rate of the device (pf_fp64_fma_peak): 8 independent DFMA chains per thread, 1024 threads per CTA, 4 CTAs per SM
+__global__ void __launch_bounds__(1024) fp64_peak_kernel(double *out, int iters, double a, double b)
+{
+    double x[8];
+#pragma unroll
+    for (int i = 0; i < 8; ++i) x[i] = 1.0 + 1e-9 * (threadIdx.x + i);
+    for (int it = 0; it < iters; ++it) {
+#pragma unroll
+        for (int i = 0; i < 8; ++i) x[i] = fma(x[i], a, b);
+    }
+    double sum = 0.0;
+#pragma unroll
+    for (int i = 0; i < 8; ++i) sum += x[i];
+    if (sum == 12345.678) out[0] = sum;            // never true: keeps the chains alive
+}
+
 // ================================================================== C ABI =========================
 extern "C" {
 
@@ -748,6 +764,35 @@ int pf_set_dt(pf_ctx *c, double dt)
 }
 
 long long pf_launch_count(const pf_ctx *c) { return c ? c->launches : 0; }
+
+int pf_fp64_fma_peak(double *tflops)
+{
+    if (!tflops) return PF_EINVAL;
+    int dev = 0, sms = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess || cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess) {
+        cudaGetLastError();
+        return PF_ECUDA;
+    }
+    double *buf = nullptr;
+    cudaEvent_t e0, e1;
+    if (cudaMalloc((void **)&buf, 64) != cudaSuccess) { cudaGetLastError(); return PF_ECUDA; }
+    cudaEventCreate(&e0); cudaEventCreate(&e1);
+    const int iters = 1 << 14, grid = sms * 4;
+    double best = 0.0;
+    for (int rep = 0; rep < 4; ++rep) {                  // first pass is the warm-up
+        cudaEventRecord(e0);
+        fp64_peak_kernel<<<grid, 1024>>>(buf, iters, 0.999999, 1e-6);
+        cudaEventRecord(e1);
+        if (cudaEventSynchronize(e1) != cudaSuccess) { cudaGetLastError(); cudaFree(buf); return PF_ECUDA; }
+        float ms = 0;
+        cudaEventElapsedTime(&ms, e0, e1);
+        const double t = 2.0 * 8.0 * iters * 1024.0 * grid / (ms * 1e-3) / 1e12;
+        if (rep > 0 && t > best) best = t;
+    }
+    cudaEventDestroy(e0); cudaEventDestroy(e1); cudaFree(buf);
+    *tflops = best;
+    return PF_OK;
+}
 
 int pf_set_profiling(pf_ctx *c, int on)
 {

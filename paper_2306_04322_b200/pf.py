@@ -20,7 +20,7 @@ PF_HOST, PF_DEVICE = 0, 1
 PF_OK, PF_EINVAL, PF_ENOMEM, PF_ECUDA, PF_ESTATE, PF_EUNSUPPORTED = 0, -1, -2, -3, -4, -5
 
 EXPORTS = ["pf_create", "pf_create_batch", "pf_batch_size", "pf_set_fields", "pf_step_fs", "pf_step_fd", "pf_get_fields", "pf_free_energy",
-           "pf_set_dt", "pf_launch_count", "pf_set_profiling", "pf_num_fs_kernels", "pf_fs_kernel_ms", "pf_launch_fs_kernel",
+           "pf_set_dt", "pf_launch_count", "pf_fp64_fma_peak", "pf_set_profiling", "pf_num_fs_kernels", "pf_fs_kernel_ms", "pf_launch_fs_kernel",
            "pf_fs_kernel_name", "pf_strerror", "pf_last_cuda_error", "pf_destroy"]
 
 
@@ -74,6 +74,8 @@ def lib() -> ctypes.CDLL:
         L.pf_set_dt.argtypes = [vp, ctypes.c_double]
         L.pf_launch_count.restype = ctypes.c_longlong
         L.pf_launch_count.argtypes = [vp]
+        L.pf_fp64_fma_peak.restype = ctypes.c_int
+        L.pf_fp64_fma_peak.argtypes = [ctypes.POINTER(ctypes.c_double)]
         L.pf_set_profiling.restype = ctypes.c_int
         L.pf_set_profiling.argtypes = [vp, ctypes.c_int]
         L.pf_num_fs_kernels.restype = ctypes.c_int
@@ -112,6 +114,15 @@ def make_params(n, n_eta=4, dx=1.0, dt=5e-3, M=5.0, L=5.0, kappa_c=3.0, kappa_et
     p.k2_kind = int(k2_kind)
     p.stream = ctypes.c_void_p(stream) if stream else None
     return p
+
+
+def fp64_fma_peak() -> float:
+    """Measured fp64 FMA rate of the current device, TFLOP/s (pf_fp64_fma_peak)."""
+    out = ctypes.c_double()
+    rc = lib().pf_fp64_fma_peak(ctypes.byref(out))
+    if rc != PF_OK:
+        raise PfError(rc, "pf_fp64_fma_peak", lib().pf_strerror(rc).decode())
+    return float(out.value)
 
 
 class Context:
