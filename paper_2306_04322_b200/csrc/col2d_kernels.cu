@@ -24,6 +24,10 @@
 #include "pf_kernels.cuh"
 #include "col_buf.cuh"
 
+#ifndef PF_COL2D_TP2048
+#define PF_COL2D_TP2048 2
+#endif
+
 namespace pf {
 
 namespace {
@@ -281,7 +285,7 @@ template <typename T, int N, int E, int TP> struct Col2dInst {
             if (nfft == 2048) return Col2dInst<T, 2048, 16, 2>::CALL;            \
         } else {                                                                 \
             if (nfft == 1024) return Col2dInst<T, 1024, 8, 2>::CALL;             \
-            if (nfft == 2048) return Col2dInst<T, 2048, 8, 2>::CALL;             \
+            if (nfft == 2048) return Col2dInst<T, 2048, 8, PF_COL2D_TP2048>::CALL; \
         }                                                                        \
         switch (nfft) {                                                          \
         case 16:   return Col2dInst<T, 16, 8, 8>::CALL;                          \
