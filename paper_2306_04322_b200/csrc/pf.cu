@@ -57,6 +57,7 @@ struct pf_ctx {
     int state = ST_NONE;
     bool s2c_valid = false;
     // 2D: carried spectrum of c and the static schedule of the last-axis kernel (col2d_kernels.cu)
+    bool legacy_fd2d = false;            // PF_FD2D_LEGACY=1: fd_fused2d_kernel for every 2D shape (A/B runs)
     bool legacy_fd3d = false;            // PF_FD3D_LEGACY=1: fd_fused3d_kernel for every 3D shape (A/B runs)
     bool legacy_col2d = false;           // PF_COL2D_LEGACY=1: the one-CTA-per-(field, block) kernel of col_kernels.cu (A/B runs)
     void *carry = nullptr;
@@ -426,7 +427,9 @@ template <typename T> int step_fd(pf_ctx *c, int nsteps)
         T *cu = (T *)c->real[c->cur], *nw = (T *)c->real[c->cur ^ 1];
         f.c = cu; f.eta = cu + c->B * c->N; f.c_new = nw; f.eta_new = nw + c->B * c->N;
         if (c->p.ndim == 2) {
-            PF_CK(c, launch_fd_fused2d<T>(f, c->stream));
+            cudaError_t e = c->legacy_fd2d ? cudaErrorNotSupported : launch_fd2d_pair<T>(f, c->stream);
+            if (e == cudaErrorNotSupported) e = launch_fd_fused2d<T>(f, c->stream);
+            PF_CK(c, e);
             c->launches += 1;
         } else {
             cudaError_t e = c->legacy_fd3d ? cudaErrorNotSupported : launch_fd3d_march<T>(f, c->stream);
@@ -605,6 +608,7 @@ static int create_impl(const pf_params *p, int nbatch, pf_ctx **out)
     c->device = dev;
     { const char *e = getenv("PF_WCOL"); c->use_wcol = (e && e[0] == '1' && nbatch == 1); }
     { const char *e = getenv("PF_COL2D_LEGACY"); c->legacy_col2d = (e && e[0] == '1' && nbatch == 1); }
+    { const char *e = getenv("PF_FD2D_LEGACY"); c->legacy_fd2d = (e && e[0] == '1'); }
     { const char *e = getenv("PF_FD3D_LEGACY"); c->legacy_fd3d = (e && e[0] == '1'); }
     { const char *e = getenv("PF_NO_GRAPH"); if (e && e[0] == '1') c->graph_ok = false; }
     if (p->ndim == 2) { c->p.n[2] = 1; c->p.dx[2] = 1.0; }

@@ -181,6 +181,8 @@ template <typename T> cudaError_t launch_col2d(int nfft, const Col2dParams<T> &p
 template <typename T> int sgrid_plan(int nx, int ny, int F, int want);
 template <typename T> cudaError_t launch_sgrid(int nx, int ny, const SgParams<T> &p, int cs, int nbatch, cudaStream_t s);
 template <typename T> cudaError_t launch_fd_fused2d(const FdParams<T> &p, cudaStream_t s);
+// 2D, nx >= 64, ny >= 16: pair-wide tile kernel (fd2d_kernels.cu); cudaErrorNotSupported otherwise
+template <typename T> cudaError_t launch_fd2d_pair(const FdParams<T> &p, cudaStream_t s);
 template <typename T> cudaError_t launch_fd_fused3d(const FdParams<T> &p, cudaStream_t s);
 // 3D, nx >= 64, at most four order parameters (fd3d_kernels.cu); cudaErrorNotSupported otherwise
 template <typename T> cudaError_t launch_fd3d_march(const FdParams<T> &p, cudaStream_t s);

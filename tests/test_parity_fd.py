@@ -107,3 +107,24 @@ def test_fd_3d_anisotropic_spacing_noise(oracle):
     dt = 0.5 * 2.0 / (5.0 * kt2 * (4.0 + 3.0 * kt2))
     (gc, geta), (rc, reta) = run_both(oracle, n=n, n_eta=2, init="A", steps=50, dt=dt, method="fd", dx=dx)
     assert rel_linf([gc, geta], [rc, reta]) < 1e-12
+
+
+@pytest.mark.parametrize("n,n_eta,steps,precision", [((64, 16), 0, 40, "f64"), ((64, 64), 8, 30, "f64"), ((128, 32), 5, 30, "f64"),
+                                                     ((256, 16), 3, 30, "f64"), ((64, 128), 1, 30, "f64"), ((128, 64), 4, 60, "f32"),
+                                                     ((64, 32), 7, 30, "f32")])
+def test_fd_2d_pair_kernel(oracle, n, n_eta, steps, precision):
+    # fd2d_kernels.cu (nx >= 64, ny >= 16: two points per thread in two rows): every field count, one tile per row / per column
+    # (the halo wraps onto the tile itself), both precisions
+    c, eta, dx = make_init("B", n, n_eta)
+    kt2 = sum(4.0 / d ** 2 for d in dx)
+    dt = min(0.75 * 2.0 / (5.0 * kt2 * (4.0 + 3.0 * kt2)), 2e-3)
+    (gc, geta), (rc, reta) = run_both(oracle, n=n, n_eta=n_eta, init="B", steps=steps, dt=dt, method="fd", precision=precision)
+    assert rel_linf([gc, geta], [rc, reta]) < (1e-12 if precision == "f64" else 1e-5)
+
+
+def test_fd_2d_pair_kernel_noise_anisotropic(oracle):
+    n, dx = (128, 64), (1.0, 0.7)
+    kt2 = sum(4.0 / d ** 2 for d in dx)
+    dt = 0.5 * 2.0 / (5.0 * kt2 * (4.0 + 3.0 * kt2))
+    (gc, geta), (rc, reta) = run_both(oracle, n=n, n_eta=2, init="A", steps=80, dt=dt, method="fd", dx=dx)
+    assert rel_linf([gc, geta], [rc, reta]) < 1e-12
