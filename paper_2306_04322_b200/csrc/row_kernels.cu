@@ -61,7 +61,9 @@ template <int M, int E> __host__ __device__ constexpr int row_pitch() { return M
 // Register cap: the kernel is bound by fp64 issue and shared-memory exchange latency, so resident warps matter more
 // than the last few registers (measured on B200: 94 -> 80 registers: 1024^2 row kernel 28.1 -> 26.4 us; 64 at
 // nx = 256: 394 -> 317 us at 256^3).
-template <typename T, int M, int E, int MODE, int REGS>
+// NF > 0: the field count as a compile-time constant (the loops over the fields of a point unroll; c + 2 eta and c + 4 eta, the
+// counts of the benchmark configurations); NF == 0: any count, from p.F
+template <typename T, int M, int E, int MODE, int REGS, int NF>
 __global__ void __maxnreg__(REGS) row_kernel(const RowParams<T> p)
 {
 #ifdef PF_DBG_EMPTY
@@ -76,13 +78,16 @@ __global__ void __maxnreg__(REGS) row_kernel(const RowParams<T> p)
     extern __shared__ __align__(16) unsigned char smem_raw[];
     C *smem = reinterpret_cast<C *>(smem_raw);
 
-    const int F = p.F;
+    const int F = NF ? NF : p.F;
     const int tid = threadIdx.x;
     const int j = tid & (TT - 1);
-    const int rf = tid / TT;
-    const int r = rf / F;
-    const int f = rf - r * F;
+    // transform `tid / TT` of the CTA is field f of row r, FIELD-major: the two or more transforms that share a warp when TT < 32
+    // then belong to the same field (RB is even there), so a warp never runs both the c branch and the eta branch of the
+    // nonlinear section
     const int RB = blockDim.x / (TT * F);
+    const int f = (tid / TT) / RB;
+    const int r = (tid / TT) - f * RB;
+    const int rf = r * F + f;                          // exchange buffer of this transform
     const long row = (long)blockIdx.x * RB + r;
     const bool valid = row < p.nrows;
     RowBuf<C, 3> buf{smem + (long)rf * MP};
@@ -163,7 +168,7 @@ __global__ void __maxnreg__(REGS) row_kernel(const RowParams<T> p)
 #endif
 }
 
-template <typename T, int M, int E, int MODE, int REGS>
+template <typename T, int M, int E, int MODE, int REGS, int NF = 0>
 static cudaError_t launch_row_inst(const RowParams<T> &p, cudaStream_t s)
 {
     typedef typename V2<T>::type C;
@@ -175,9 +180,10 @@ static cudaError_t launch_row_inst(const RowParams<T> &p, cudaStream_t s)
     if (RB > p.nrows / 296) RB = p.nrows / 296;      // small grids: at least two CTAs per SM before rows are batched
     if (RB < 1) RB = 1;
     if (RB > p.nrows) RB = p.nrows;
+    if (TT < 32 && RB >= 32 / TT) RB -= RB % (32 / TT);          // whole warps per field (see the kernel)
     const int threads = RB * per_row;
     const size_t smem = (size_t)RB * p.F * row_pitch<M, E>() * sizeof(C);
-    auto kern = row_kernel<T, M, E, MODE, REGS>;
+    auto kern = row_kernel<T, M, E, MODE, REGS, NF>;
     if (smem > 48 * 1024) {
         cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
         if (e != cudaSuccess) return e;
@@ -195,7 +201,10 @@ static cudaError_t launch_row_mode(int mode, const RowParams<T> &p, cudaStream_t
 {
     switch (mode) {
     case ROW_SET:  return launch_row_inst<T, M, E, ROW_SET, REGS>(p, s);
-    case ROW_STEP: return launch_row_inst<T, M, E, ROW_STEP, REGS>(p, s);
+    case ROW_STEP:
+        if (p.F == 3) return launch_row_inst<T, M, E, ROW_STEP, REGS, 3>(p, s);
+        if (p.F == 5) return launch_row_inst<T, M, E, ROW_STEP, REGS, 5>(p, s);
+        return launch_row_inst<T, M, E, ROW_STEP, REGS>(p, s);
     case ROW_GET:  return launch_row_inst<T, M, E, ROW_GET, REGS>(p, s);
     }
     return cudaErrorInvalidValue;
