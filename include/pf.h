@@ -93,8 +93,8 @@ int pf_set_fields(pf_ctx *ctx, const void *c, const void *eta, int where);
  * with |xi|^2 of k2_kind. The fields are kept in a partially transformed form between steps; the
  * real fields are materialised by pf_get_fields / pf_step_fd / pf_free_energy.
  * Launches: 2 (2D) or 4 (3D) kernels per step, replayed as a CUDA graph of 8 steps for calls of at least 8 steps; square 2D
- * grids up to 64 x 64 run ALL steps of the call in ONE launch (state resident in the shared memory of a thread-block cluster),
- * so one call of n steps is much cheaper there than n calls of one step.
+ * grids up to 64 x 64 run ALL steps of a call of two or more steps in ONE launch (state resident in the shared memory of a
+ * thread-block cluster), so one call of n steps is much cheaper there than n calls of one step.
  * nsteps == 0 is a no-op; nsteps < 0 -> PF_EINVAL; no fields set -> PF_ESTATE.
  * Non-finite values are not an error (they propagate). */
 int pf_step_fs(pf_ctx *ctx, int nsteps);
