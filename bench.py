@@ -97,7 +97,7 @@ def kernel_source_hash():
     h = hashlib.sha256()
     d = os.path.join(ROOT, "paper_2306_04322_b200", "csrc")
     for f in sorted(os.listdir(d)):
-        if f.endswith((".cu", ".cuh")):
+        if f.endswith(".cuh") or f.endswith("_kernels.cu"):         # kernels only: pf.cu is host code
             h.update(open(os.path.join(d, f), "rb").read())
     return h.hexdigest()[:16]
 
