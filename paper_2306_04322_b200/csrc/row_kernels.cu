@@ -34,6 +34,9 @@
 // 1024 threads at F = 9), so these run 16 elements per thread: F * 64 <= 576 threads = 18 warps, i.e. up to 5 warps on one
 // of the four 16 K-register sub-partitions -> at most 102 registers per thread
 #define PF_ROW_REGS_WIDE 96
+#ifndef PF_ROW_LOGPAD
+#define PF_ROW_LOGPAD(C) (sizeof(C) == 8 ? 4 : 3)
+#endif
 
 namespace pf {
 
@@ -72,6 +75,9 @@ __global__ void __maxnreg__(REGS) row_kernel(const RowParams<T> p)
     typedef typename V2<T>::type C;
     constexpr int TT = M / E;
     constexpr int MP = row_pitch<M, E>();
+    // one element of padding per 128-byte line of the exchange buffer: 8 fp64 / 16 fp32 complex values (with one per 8 the
+    // first-stage scatter of the fp32 transforms ran at twice the minimum number of wavefronts, profiles/r2_ncu_full.md)
+    constexpr int LP = PF_ROW_LOGPAD(C);
 #ifdef PF_TRACE
     TraceScope trace(p.trace, 0);
 #endif
@@ -90,7 +96,7 @@ __global__ void __maxnreg__(REGS) row_kernel(const RowParams<T> p)
     const int rf = r * F + f;                          // exchange buffer of this transform
     const long row = (long)blockIdx.x * RB + r;
     const bool valid = row < p.nrows;
-    RowBuf<C, 3> buf{smem + (long)rf * MP};
+    RowBuf<C, LP> buf{smem + (long)rf * MP};
     const CtaSync sync;
     const int rf_sync = threadIdx.x / TT;              // transform index within the CTA (at most 9 when TT > 32)
 
@@ -132,7 +138,7 @@ __global__ void __maxnreg__(REGS) row_kernel(const RowParams<T> p)
 #pragma unroll
         for (int q = 0; q < E; ++q) {
             const int n = j + q * TT;
-            const int np = n + (n >> 3);
+            const int np = n + (n >> LP);
             if (f == 0) {
                 T h0 = 0, h1 = 0;                        // h(eta) = sum_i eta_i^3 (6 eta_i^2 - 15 eta_i + 10)
                 for (int ff = 1; ff < F; ++ff) {

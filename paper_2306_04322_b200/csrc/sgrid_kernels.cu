@@ -110,7 +110,7 @@ __global__ void __launch_bounds__(SgShape<M, NY>::NT, 1) sgrid_kernel(const SgPa
     const T sM = T(1) / T(M), sN = T(1) / T(NY);
     // x transforms: lane -> (row unit of this pass, j)
     const int xu = lane / TTX, xj = lane % TTX;
-    SgRowBuf<C, 3> rbuf{scr + xu * Sh::ROWPITCH};
+    SgRowBuf<C, (sizeof(C) == 8 ? 4 : 3)> rbuf{scr + xu * Sh::ROWPITCH};   // one pad element per 128-byte line
     // y transforms: lane -> (column slot, j); slot = pair * 2 + side, the slot is the fastest index
     const int sl = lane % SLOTS, side = sl & 1, yj = lane / SLOTS;
     ColBuf<C, SLOTS, Sh::LR> cbuf{scr, sl};
