@@ -64,8 +64,8 @@ template <int M, int E> __host__ __device__ constexpr int row_pitch() { return M
 // Register cap: the kernel is bound by fp64 issue and shared-memory exchange latency, so resident warps matter more
 // than the last few registers (measured on B200: 94 -> 80 registers: 1024^2 row kernel 28.1 -> 26.4 us; 64 at
 // nx = 256: 394 -> 317 us at 256^3).
-// NF > 0: the field count as a compile-time constant (the loops over the fields of a point unroll; c + 2 eta and c + 4 eta, the
-// counts of the benchmark configurations); NF == 0: any count, from p.F
+// NF > 0: the field count as a compile-time constant (the loops over the fields of a point unroll); NF == 0: from p.F (ROW_SET / ROW_GET,
+// which do not loop over fields)
 template <typename T, int M, int E, int MODE, int REGS, int NF>
 __global__ void __maxnreg__(REGS) row_kernel(const RowParams<T> p)
 {
@@ -208,8 +208,17 @@ static cudaError_t launch_row_mode(int mode, const RowParams<T> &p, cudaStream_t
     switch (mode) {
     case ROW_SET:  return launch_row_inst<T, M, E, ROW_SET, REGS>(p, s);
     case ROW_STEP:
-        if (p.F == 3) return launch_row_inst<T, M, E, ROW_STEP, REGS, 3>(p, s);
-        if (p.F == 5) return launch_row_inst<T, M, E, ROW_STEP, REGS, 5>(p, s);
+        switch (p.F) {                     // field count as a template parameter (see the kernel)
+        case 1: return launch_row_inst<T, M, E, ROW_STEP, REGS, 1>(p, s);
+        case 2: return launch_row_inst<T, M, E, ROW_STEP, REGS, 2>(p, s);
+        case 3: return launch_row_inst<T, M, E, ROW_STEP, REGS, 3>(p, s);
+        case 4: return launch_row_inst<T, M, E, ROW_STEP, REGS, 4>(p, s);
+        case 5: return launch_row_inst<T, M, E, ROW_STEP, REGS, 5>(p, s);
+        case 6: return launch_row_inst<T, M, E, ROW_STEP, REGS, 6>(p, s);
+        case 7: return launch_row_inst<T, M, E, ROW_STEP, REGS, 7>(p, s);
+        case 8: return launch_row_inst<T, M, E, ROW_STEP, REGS, 8>(p, s);
+        case 9: return launch_row_inst<T, M, E, ROW_STEP, REGS, 9>(p, s);
+        }
         return launch_row_inst<T, M, E, ROW_STEP, REGS>(p, s);
     case ROW_GET:  return launch_row_inst<T, M, E, ROW_GET, REGS>(p, s);
     }
