@@ -237,22 +237,52 @@ col_kernel(const ColParams<T> p)
     grid_dependents_launch();
 
     C *park = nullptr;
+    bool carried = false;
     if (c_cta) {
-        // Cahn-Hilliard needs two transforms on the same columns: dt M |xi|^2 g^ is formed first and parked in
-        // global memory (thread-linear: written and read back by the same thread, L2 resident), then c^ follows.
+        // thread-linear scratch of this CTA's columns: written and read back by the same thread
         park = p.park + ((bz * gridDim.x + ub) * (long)E) * GT + tid;
+        if (p.has_c == 3) {
+            // one-off (after pf_set_fields / FD steps): the carried spectrum c^ = FFT of the columns of c
+            load_columns(p.in0 + bz * p.in_bs);
+            forward(v);
+#pragma unroll
+            for (int q = 0; q < E; ++q) park[(long)q * GT] = v[q];
+            return;
+        }
         load_columns(in);
         forward(v);
+        if (p.has_c == 2) {
+            // c^ is CARRIED in the scratch array, as Algorithm 1 carries it: the Cahn-Hilliard columns cost
+            // two transforms (g^, inverse) instead of three and nothing is parked
+            //   c^ <- (c^ - dt M |xi|^2 g^) / (1 + dt M kappa_c |xi|^4)                           Eqs. 12, 14
+            const T s = T(1) / T(N);
 #pragma unroll
-        for (int q = 0; q < E; ++q) park[(long)q * GT] = cscale(v[q], p.m.dtM * (base2 + klast[kq(q)]));
-        in = p.in0 + bz * p.in_bs;
+            for (int q = 0; q < E; ++q) {
+                const T k2 = base2 + klast[kq(q)];
+                const T d = rcp(T(1) + p.m.dtMkc * k2 * k2);
+                const T a = p.m.dtM * k2;
+                const C cq = park[(long)q * GT];
+                const C cn = mk<T>((cq.x - a * v[q].x) * d, (cq.y - a * v[q].y) * d);
+                park[(long)q * GT] = cn;
+                v[q] = cscale(cn, s);
+            }
+            carried = true;
+        } else {
+            // Cahn-Hilliard with two forward transforms on the same columns: dt M |xi|^2 g^ is formed first and parked in
+            // global memory (L2 resident), then c^ follows (2D legacy kernel, PF_COL3D_PARK=1)
+#pragma unroll
+            for (int q = 0; q < E; ++q) park[(long)q * GT] = cscale(v[q], p.m.dtM * (base2 + klast[kq(q)]));
+            in = p.in0 + bz * p.in_bs;
+        }
     }
 
-    load_columns(in);
-    if (DO_FWD) forward(v);
+    if (!carried) {
+        load_columns(in);
+        if (DO_FWD) forward(v);
+    }
 
 #ifndef PF_DBG_SKIP_UPDATE
-    if (DO_UPD) {
+    if (DO_UPD && !carried) {
         const T s = T(1) / T(N);
         if (c_cta) {
 #pragma unroll

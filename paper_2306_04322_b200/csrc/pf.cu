@@ -57,6 +57,7 @@ struct pf_ctx {
     int state = ST_NONE;
     bool s2c_valid = false;
     // 2D: carried spectrum of c and the static schedule of the last-axis kernel (col2d_kernels.cu)
+    bool park3d = false;                 // PF_COL3D_PARK=1: 3D z kernel re-transforms c every step (round-1 form, A/B runs)
     bool legacy_fd2d = false;            // PF_FD2D_LEGACY=1: fd_fused2d_kernel for every 2D shape (A/B runs)
     bool legacy_fd3d = false;            // PF_FD3D_LEGACY=1: fd_fused3d_kernel for every 3D shape (A/B runs)
     bool legacy_col2d = false;           // PF_COL2D_LEGACY=1: the one-CTA-per-(field, block) kernel of col_kernels.cu (A/B runs)
@@ -290,7 +291,7 @@ template <typename T> int fs_one_step(pf_ctx *c, cudaEvent_t *events, int only =
             q.tw = (const C *)c->tw_z;
             q.in_rs = q.out_rs = (long)ny * c->P2; q.ncols = ny * c->P2;
             q.in0 = s2; q.in1 = (const C *)c->g2; q.out = s2; q.in_fs = q.out_fs = s2fs;
-            q.has_c = 1; q.pdl = pdl;
+            q.has_c = c->park3d ? 1 : 2; q.pdl = pdl;          // 2: c^ carried in `park` (filled by to_spectral)
             PF_CK(c, launch_col<T>(COL_3D_LAST, nz, c->F, 1, q, c->stream)); ++c->launches;
         }
         kt.mark("col_z_fft_update_ifft");
@@ -321,7 +322,19 @@ template <typename T> int to_spectral(pf_ctx *c, bool need_carry = true)
         c->carry_valid = true;
     }
     if (c->p.ndim == 3 && !c->s2c_valid) {
+        typedef typename V2<T>::type C;
         PF_CK(c, mid_forward<T>(c, c->zst, 0, c->s2, 0, 1, false, false));
+        if (!c->park3d) {
+            // the carried spectrum c^ of the z kernel, in its thread-linear order (same launch geometry, slot 0 only)
+            const int ny = c->p.n[1], nz = c->p.n[2];
+            ColParams<T> q = col_params<T>(c);
+            q.tw = (const C *)c->tw_z;
+            q.in_rs = q.out_rs = (long)ny * c->P2; q.ncols = ny * c->P2;
+            q.in0 = (const C *)c->s2; q.in1 = (const C *)c->g2; q.out = (C *)c->s2;
+            q.in_fs = q.out_fs = (long)nz * ny * c->P2;
+            q.has_c = 3; q.pdl = 0;
+            PF_CK(c, launch_col<T>(COL_3D_LAST, nz, 1, 1, q, c->stream)); ++c->launches;
+        }
         c->s2c_valid = true;
     }
     return PF_OK;
@@ -609,6 +622,7 @@ static int create_impl(const pf_params *p, int nbatch, pf_ctx **out)
     c->device = dev;
     { const char *e = getenv("PF_WCOL"); c->use_wcol = (e && e[0] == '1' && nbatch == 1); }
     { const char *e = getenv("PF_COL2D_LEGACY"); c->legacy_col2d = (e && e[0] == '1' && nbatch == 1); }
+    { const char *e = getenv("PF_COL3D_PARK"); c->park3d = (e && e[0] == '1'); }
     { const char *e = getenv("PF_FD2D_LEGACY"); c->legacy_fd2d = (e && e[0] == '1'); }
     { const char *e = getenv("PF_FD3D_LEGACY"); c->legacy_fd3d = (e && e[0] == '1'); }
     { const char *e = getenv("PF_NO_GRAPH"); if (e && e[0] == '1') c->graph_ok = false; }

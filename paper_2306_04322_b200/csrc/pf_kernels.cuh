@@ -86,7 +86,8 @@ template <typename T> struct ColParams {
     C       *park;           // update modes with has_c: scratch for dt M |xi|^2 g^, one complex per spectral mode (+ padding)
     const C *alt_in;         // if non-null, slot 0 reads alt_in and writes alt_out instead (3D y-forward of g)
     C       *alt_out;
-    int      has_c;          // update modes: slot 0 is the Cahn-Hilliard field (needs in1)
+    int      has_c;          // update modes: slot 0 is the Cahn-Hilliard field (needs in1). 1: c^ re-transformed, dt M |xi|^2 g^ parked;
+                             // 2: c^ carried in `park`; 3: one-off pass that fills the carried spectrum from in0 (slot 0 only)
     int      pdl;            // launch with programmatic stream serialization
     long     in_fs, out_fs;  // slot strides (blockIdx.z)
     long     in_bs, out_bs;           // batch strides (blockIdx.y; 3D mid kernels: z planes)
