@@ -114,6 +114,43 @@ int pf_get_fields(pf_ctx *ctx, void *c, void *eta, int where);
  * gradient_kind 1: forward differences (the discretisation the 5/7-point Laplacian derives from). */
 int pf_free_energy(pf_ctx *ctx, int gradient_kind, double *out);
 
+/* Free energy for callers that must not allocate device memory.
+ *
+ * pf_free_energy needs a context, and pf_create pays for a context with a dozen cudaMalloc calls. That rules it out for
+ * code that runs where allocating is not an option: a plug-in inside an application whose own memory pool already owns
+ * (almost) all of the device, so that a further cudaMalloc fails or takes memory the plug-in has no claim to; an in-situ
+ * energy monitor called from another solver's time loop, where cudaMalloc/cudaFree would stall the device on every call;
+ * any program with a "nothing is allocated after start-up" rule. pf_free_energy_static serves those callers: no
+ * context, no cudaMalloc/cudaFree or other allocating call, ever. Its working memory (per-tile partial sums, a ticket,
+ * the result) is a fixed array compiled into libpf.so -- PF_STATIC_SCRATCH_BYTES of global memory that every GPU which
+ * loads the library holds until the process exits. The price is a size limit and one shared array.
+ *
+ * Computes Eq. 1 exactly as pf_free_energy(ctx, gradient_kind = 1, out) does -- f_chem of PAPER.md:46,
+ * forward-difference gradients with periodic wrap-around, Riemann sum with cell volume prod(dx), fp64 accumulation --
+ * for fields the caller already has on the device.
+ *   p    read: ndim, n, n_eta, dx, kappa_c, kappa_eta, rho2, c_alpha, c_beta, w, alpha, precision, stream; the rest
+ *        (dt, M, L, k2_kind) is ignored. stream NULL = the legacy default stream;
+ *   c    DEVICE pointer (current device), [nz][ny][nx] of float/double per p->precision; read only, caller keeps it;
+ *   eta  DEVICE pointer, [n_eta][nz][ny][nx]; may be NULL iff n_eta == 0;
+ *   out  HOST pointer, 3 + n_eta doubles: total, chemical, kappa_c/2 |grad c|^2, kappa_eta/2 |grad eta_i|^2 ...
+ * The call queues one memset and one kernel on p->stream, copies the result out and returns after that stream has
+ * drained. The sum is taken tile by tile in a fixed order: the same input gives the same bits on every run.
+ * Limits: at most PF_STATIC_MAX_POINTS grid points (nx*ny*nz; 2048^2 and 256^3 fit, 512^3 does not) and n_eta <= 8;
+ *   grid sizes as for pf_create. A grid beyond the limit is refused with PF_EUNSUPPORTED before anything is queued --
+ *   use a context and pf_free_energy for those.
+ * Sharing: there is one array per GPU, shared by every call in the process. It keeps the previous call's contents; the
+ *   slots that must start at zero are cleared at the head of each call. Calls whose GPU work can overlap (two streams,
+ *   two host threads) race on it and return garbage -- issue them on one stream or serialise them yourself.
+ * First call on a device: looks up the device address of the array (cudaGetSymbolAddress, with that device current)
+ *   and remembers it; make that first call during start-up, before any stream capture is begun.
+ * PF_EINVAL: null pointers, bad ndim / n_eta / precision / dx, c or eta not device memory of the current device;
+ * PF_EUNSUPPORTED: grid not a power of two in 16..2048 per axis, or more than PF_STATIC_MAX_POINTS points;
+ * PF_ECUDA: no usable device or a CUDA call failed. */
+#define PF_STATIC_TILE          4096                        /* grid points summed by one CTA                  */
+#define PF_STATIC_MAX_POINTS    (1 << 24)                   /* 4096 tiles                                      */
+#define PF_STATIC_SCRATCH_BYTES ((32 + 4096 * 10) * 8)      /* 327 936 bytes held per GPU for the process' life */
+int pf_free_energy_static(const pf_params *p, const void *c, const void *eta, double *out);
+
 /* Changes dt for subsequent steps (the dt sweep of the FS-vs-FD crossover); dt <= 0 -> PF_EINVAL. */
 int pf_set_dt(pf_ctx *ctx, double dt);
 

@@ -20,7 +20,7 @@ CSRC = os.path.join(HERE, "csrc")
 SUFFIX = os.environ.get("PF_BUILD_SUFFIX", "")
 OBJ = os.path.join(HERE, "csrc", "build" + ("_" + SUFFIX if SUFFIX else ""))
 SO = os.path.join(HERE, "libpf" + ("_" + SUFFIX if SUFFIX else "") + ".so")
-UNITS = ["row_kernels", "col_kernels", "col2d_kernels", "wcol_kernels", "fd_kernels", "fd2d_kernels", "fd3d_kernels", "sgrid_kernels", "pf"]
+UNITS = ["row_kernels", "col_kernels", "col2d_kernels", "wcol_kernels", "fd_kernels", "fd2d_kernels", "fd3d_kernels", "sgrid_kernels", "static_energy", "pf"]
 HEADERS = sorted(glob.glob(os.path.join(CSRC, "*.cuh"))) + [os.path.join(os.path.dirname(HERE), "include", "pf.h")]
 NVCC_FLAGS = ["-std=c++17", "-O3", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo",
               "-Xcompiler", "-fPIC", "-Xptxas", "-v"] + os.environ.get("PF_EXTRA_NVCC_FLAGS", "").split()

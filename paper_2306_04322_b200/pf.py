@@ -20,7 +20,7 @@ PF_HOST, PF_DEVICE = 0, 1
 PF_OK, PF_EINVAL, PF_ENOMEM, PF_ECUDA, PF_ESTATE, PF_EUNSUPPORTED = 0, -1, -2, -3, -4, -5
 
 EXPORTS = ["pf_create", "pf_create_batch", "pf_batch_size", "pf_set_fields", "pf_step_fs", "pf_step_fd", "pf_get_fields", "pf_free_energy",
-           "pf_set_dt", "pf_launch_count", "pf_fp64_fma_peak", "pf_set_profiling", "pf_num_fs_kernels", "pf_fs_kernel_ms", "pf_launch_fs_kernel",
+           "pf_free_energy_static", "pf_set_dt", "pf_launch_count", "pf_fp64_fma_peak", "pf_set_profiling", "pf_num_fs_kernels", "pf_fs_kernel_ms", "pf_launch_fs_kernel",
            "pf_fs_kernel_name", "pf_strerror", "pf_last_cuda_error", "pf_destroy"]
 
 
@@ -70,6 +70,8 @@ def lib() -> ctypes.CDLL:
         L.pf_step_fd.argtypes = [vp, ctypes.c_int]
         L.pf_free_energy.restype = ctypes.c_int
         L.pf_free_energy.argtypes = [vp, ctypes.c_int, ctypes.POINTER(ctypes.c_double)]
+        L.pf_free_energy_static.restype = ctypes.c_int
+        L.pf_free_energy_static.argtypes = [pp, vp, vp, ctypes.POINTER(ctypes.c_double)]
         L.pf_set_dt.restype = ctypes.c_int
         L.pf_set_dt.argtypes = [vp, ctypes.c_double]
         L.pf_launch_count.restype = ctypes.c_longlong
@@ -123,6 +125,25 @@ def fp64_fma_peak() -> float:
     if rc != PF_OK:
         raise PfError(rc, "pf_fp64_fma_peak", lib().pf_strerror(rc).decode())
     return float(out.value)
+
+
+STATIC_MAX_POINTS = 1 << 24          # PF_STATIC_MAX_POINTS of pf.h
+
+
+def free_energy_static(c, eta, n, **kw):
+    """pf_free_energy_static: Eq. 1 with forward-difference gradients for fields that already sit on the device, for
+    callers that may not allocate device memory (an application whose own pool owns the GPU, a monitor inside another
+    solver's time loop, a no-allocation-after-start-up service). No context is created and the library allocates nothing:
+    its working memory is a fixed array inside libpf.so, shared by all calls, which is why at most STATIC_MAX_POINTS grid
+    points are accepted and why calls that overlap on the GPU must be serialised by the caller (see pf.h).
+    c, eta: objects with data_ptr() (torch CUDA tensors of the dtype `precision` names; eta may be None when n_eta == 0);
+    n and the keywords as for make_params. Returns the 3 + n_eta doubles of pf_free_energy(gradient_kind=1)."""
+    p = make_params(n, **kw)
+    out = (ctypes.c_double * (3 + p.n_eta))()
+    rc = lib().pf_free_energy_static(ctypes.byref(p), c.data_ptr(), eta.data_ptr() if p.n_eta else None, out)
+    if rc != PF_OK:
+        raise PfError(rc, "pf_free_energy_static", lib().pf_strerror(rc).decode())
+    return np.array(out[:], dtype=np.float64)
 
 
 class Context:
