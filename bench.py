@@ -8,7 +8,7 @@ the spectral update) of one simulation. At the L2-resident sizes the timed loop 
 replicas of the simulation so that consecutive steps never find their inputs in L2 (timing rule "inputs larger than
 L2"). The timed region of K steps is repeated B >= 5 times; `value` is the median batch.
 Prints ONE JSON line: the headline workload (1024sq, the metric's 2D size) at the top level and the metric's other
-size (256cube) measured in the same invocation under "workloads".
+size (256cube), configs[2] (2048sq, 2048sq_f32) and configs[1]'s grid (512sq) measured in the same invocation under "workloads".
 
 --gpus N > 1 outside torchrun re-executes itself under torch.distributed.run with N ranks (replicas only, no
 data-path collective).
@@ -74,45 +74,61 @@ def bytes_model(n, p, w):
     survey: SURVEY 8(d): one read + one write of every field per 1-D pass + the u^ read of the update, attributed to the
             kernel that performs the pass: x kernel (a6 + a1 + a2) 2F(R+S); 2D y kernel (a4 + a5) 5FS;
             3D y-forward (a3) 2FS, z kernel (a4 + a5) 5FS, y-inverse (a5) 2FS.  Sum: 2D F(2R+7S), 3D F(2R+11S).
-    design: what the kernels of this design have to move (z-form state, cross-step fusion, g^ parked in L2)."""
+    design: what the kernels of this design have to move (z-form state, cross-step fusion, c^ carried between steps as in
+            Algorithm 1): the last-axis kernel reads g^ and the carried c^, writes the carried c^ and the z-form of c (4 arrays)
+            and reads + writes every eta (2p arrays): (4 + 2p) R in 2D, (4 + 2p) Sp in 3D. Where the schedule splits a
+            Cahn-Hilliard block over two CTAs (C_FWD / C_INV) the carried c^ is read once more: at most one array on top
+            (design_upper)."""
     F = p + 1
     N = int(np.prod(n))
     R = N * w
     S = (n[0] // 2 + 1) * (N // n[0]) * 2 * w
     if len(n) == 2:
         survey = {"row_c2r_nonlinear_r2c": 2 * F * (R + S), "col_y_fft_update_ifft": 5 * F * S}
-        design = {"row_c2r_nonlinear_r2c": 2 * F * R, "col_y_fft_update_ifft": (3 + 2 * p) * R}
+        design = {"row_c2r_nonlinear_r2c": 2 * F * R, "col_y_fft_update_ifft": (4 + 2 * p) * R}
     else:
         P2 = ((n[0] // 2 + 1 + 15) // 16) * 16
         Sp = P2 * n[1] * n[2] * 2 * w          # one padded half-spectrum array as stored
         survey = {"row_c2r_nonlinear_r2c": 2 * F * (R + S), "col_y_fwd": 2 * F * S, "col_z_fft_update_ifft": 5 * F * S,
                   "col_y_inv": 2 * F * S}
         design = {"row_c2r_nonlinear_r2c": 2 * F * R, "col_y_fwd": F * (R + Sp),
-                  "col_z_fft_update_ifft": (3 + 2 * p) * Sp, "col_y_inv": F * (Sp + R)}
+                  "col_z_fft_update_ifft": (4 + 2 * p) * Sp, "col_y_inv": F * (Sp + R)}
     return survey, design
 
 
-def kernel_source_hash():
-    """Hash of the kernel sources: the ncu traffic figures under profiles/ are only quoted for the build they were taken from."""
-    h = hashlib.sha256()
-    d = os.path.join(ROOT, "paper_2306_04322_b200", "csrc")
-    for f in sorted(os.listdir(d)):
-        if f.endswith(".cuh") or f.endswith("_kernels.cu"):         # kernels only: pf.cu is host code
-            h.update(open(os.path.join(d, f), "rb").read())
-    return h.hexdigest()[:16]
+def kernel_source_hash(kernel=None):
+    """Hash of the sources a kernel is built from (kernel=None: of every kernel file). An ncu traffic figure under profiles/
+    is quoted only while the files of ITS kernel still hash to the value the capture step stored beside it."""
+    from paper_2306_04322_b200 import ncu_traffic as nt
+    return nt.source_hash(kernel)
 
 
 def ncu_traffic(workload, kernel):
     """dram__bytes_read.sum + dram__bytes_write.sum per launch from the committed ncu --set full summary
-    (profiles/ncu_traffic.json, written from the capture named in it). None when the kernel sources have changed since."""
+    (profiles/ncu_traffic.json; entries are written by `python -m paper_2306_04322_b200.ncu_traffic`, never by hand).
+    None when the sources of that kernel have changed since its capture."""
     try:
         with open(os.path.join(ROOT, "profiles", "ncu_traffic.json")) as fh:
             t = json.load(fh)
-        if t.get("kernel_source_hash") != kernel_source_hash():
-            return None, f"profiles/ncu_traffic.json was captured from other kernel sources ({t.get('kernel_source_hash')})"
-        return t["traffic"].get(workload, {}).get(kernel), t.get("capture")
+        ent = t["traffic"].get(workload, {}).get(kernel)
+        if not isinstance(ent, dict):
+            return None, "no capture of this kernel for this workload in profiles/ncu_traffic.json"
+        if ent.get("source_hash") != kernel_source_hash(kernel):
+            return None, f"profiles/ncu_traffic.json: captured from other sources of this kernel ({ent.get('source_hash')})"
+        return ent["dram_bytes_per_launch"], ent.get("capture", t.get("capture"))
     except Exception as e:
         return None, f"no profiles/ncu_traffic.json ({type(e).__name__})"
+
+
+# environment variables that make pf_create pick other kernels or launch paths (A/B runs; DESIGN.md section 8)
+SWITCHES = ["PF_WCOL", "PF_COL2D_LEGACY", "PF_COL2D_NOTICKET", "PF_COL3D_PARK", "PF_FD2D_LEGACY", "PF_FD3D_LEGACY", "PF_NO_GRAPH",
+            "PF_RESIDENT", "PF_SG_CLUSTER"]
+
+
+def live_switches():
+    """Every PF_* variable of the environment (name -> value) and the subset that changes the code path."""
+    seen = {k: v for k, v in sorted(os.environ.items()) if k.startswith("PF_")}
+    return seen, [k for k in seen if k in SWITCHES]
 
 
 class ClockSampler:
@@ -367,8 +383,8 @@ def measure_workload(wl, K, W, env, full=True):
         return replicas.max_over_ranks(e0.elapsed_time(e1), device="cuda")
 
     def fs_steps(k, which):
-        for s in range(k):                     # one step of each replica in turn; a call is asynchronous (graph replay)
-            which[s % len(which)].step_fs(1)
+        for s in range(k):                     # one step of each replica in turn: asynchronous plain launches (programmatic
+            which[s % len(which)].step_fs(1)   # stream serialization); pf_step_fs replays its graph only for calls of >= 8 steps
 
     nbatch = max(5, min(50, int(np.ceil(1000 / K))))
     fs_steps(max(W, 3) * len(ctxs), ctxs)
@@ -385,6 +401,13 @@ def measure_workload(wl, K, W, env, full=True):
     # single simulation, state resident in L2 where it fits (reported, not the headline)
     res_b = [timed(lambda: fs_steps(K, ctxs[:1])) for _ in range(5)]
     resident = replicas.job_throughput(K, stats(res_b)["median"], world)
+
+    # the launch path a long run takes: ONE pf_step_fs(K8) call on one simulation = replays of the captured 8-step graph
+    # (pf.h), beside the same simulation advanced by K8 single-step calls (plain launches) above
+    K8 = max(8, (K // 8) * 8)
+    ctxs[0].step_fs(8)
+    gr_b = [timed(lambda: ctxs[0].step_fs(K8)) for _ in range(5)]
+    graph_replay = replicas.job_throughput(K8, stats(gr_b)["median"], world)
 
     # per-kernel device times, L2-cold like the step: kernel k of every replica in turn (pf_launch_fs_kernel) between two
     # events on the stream, repeated; the replicas' fields are no trajectory afterwards (they are set again below)
@@ -415,7 +438,8 @@ def measure_workload(wl, K, W, env, full=True):
                 "frac_vs_design_bytes": kdesign[dom] / (kms[dom] * 1e-3) / 1e9 / peak,
                 "kernel_ms": kms[dom], "kernels_ms": kms,
                 "kernel_timing": f"CUDA events on the launch stream around {rounds * len(ctxs)} launches of this kernel alone, "
-                                 f"one per replica in turn ({len(ctxs)} replicas: L2-cold like the step), plain launches",
+                                 f"one per replica in turn ({len(ctxs)} replicas: L2-cold like the step), launched as in a step "
+                                 f"(programmatic stream serialization: prologues overlap the previous launch's tail)",
                 "kernel_share_of_step": kms[dom] / sum(kms.values())}
     if roofline["frac"] > 1.0:
         roofline["note"] = ("frac > 1 on the SURVEY 8(d) per-pass bytes: this kernel fuses passes whose intermediate results never "
@@ -439,7 +463,11 @@ def measure_workload(wl, K, W, env, full=True):
                               "note": "value = the median batch; every batch is K steps bracketed by barrier + synchronize, CUDA events on the launch stream, max over ranks"},
             "gpoint_updates_per_s": value * N / 1e9,
             "field_point_updates_per_s_G": value * N * F / 1e9,
-            "l2_resident_single_simulation": {"value": resident, "unit": "steps/s", "gpoint_updates_per_s": resident * N / 1e9},
+            "l2_resident_single_simulation": {"value": resident, "unit": "steps/s", "gpoint_updates_per_s": resident * N / 1e9,
+                                              "how": "one simulation, K calls of pf_step_fs(1): plain launches"},
+            "graph_replay_single_simulation": {"value": graph_replay, "unit": "steps/s", "steps_per_call": K8,
+                                               "how": "the same simulation, ONE pf_step_fs(K8) call per batch: replays of the 8-step CUDA graph "
+                                                      "(2D grids up to 64^2: the cluster-resident kernel instead)"},
             "roofline": roofline, "step_roofline": step_roofline, "gpu_launches": int(launches), "clocks": clocks}
 
     # end to end through the C ABI with HOST buffers: set (H2D) + 1 step + get (D2H), pinned host memory, ONE simulation
@@ -637,6 +665,10 @@ def run_ours(args):
     local = int(os.environ.get("LOCAL_RANK", "0"))
     if os.environ.get("PF_LIBPF") and not args.allow_lib_override:
         raise SystemExit("PF_LIBPF is set: bench.py times the product library only (ablation builds: --allow-lib-override)")
+    seen, live = live_switches()
+    if live and not args.allow_switches:
+        raise SystemExit(f"{', '.join(live)} set in the environment: these pick other kernels / launch paths than the product's "
+                         "defaults; bench.py times the defaults only (A/B runs: --allow-switches)")
     if not torch.cuda.is_available():
         raise SystemExit("bench.py needs a CUDA device (there is no CPU fallback)")
     torch.cuda.set_device(local)
@@ -652,7 +684,8 @@ def run_ours(args):
         line["fp64_fma_peak_tflops"] = {"measured": pf.fp64_fma_peak(),
                                         "nominal_from_unit_counts": 148 * 64 * 2 * 1.965e9 / 1e12,
                                         "how": "pf_fp64_fma_peak: independent DFMA chains, 4 x 1024 threads per SM, best of 3 launches"}
-    line["library"] = {"path": pf.SO_PATH, "override": bool(os.environ.get("PF_LIBPF")), "kernel_source_hash": kernel_source_hash()}
+    line["library"] = {"path": pf.SO_PATH, "override": bool(os.environ.get("PF_LIBPF")), "kernel_source_hash": kernel_source_hash(),
+                       "switches": seen, "switches_changing_the_code_path": live}
 
     if rank == 0 and world == 1 and args.workload == "1024sq" and not args.no_small_grids:
         line["small_grids"] = small_grid_measurements(env)
@@ -686,15 +719,16 @@ def main():
     ap.add_argument("--workload", default="1024sq", choices=sorted(WORKLOADS))
     ap.add_argument("--also", nargs="*", default=None, choices=sorted(WORKLOADS),
                     help="further workloads measured in the same invocation and reported under 'workloads' "
-                         "(default: 256cube beside the default headline, none otherwise)")
+                         "(default: 256cube, 2048sq, 2048sq_f32 and 512sq beside the default headline, none otherwise)")
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-cufft", action="store_true", help="skip the cuFFT side reference")
     ap.add_argument("--no-small-grids", action="store_true", help="skip the 64^2 single-simulation / batch measurements")
     ap.add_argument("--allow-lib-override", action="store_true", help="accept PF_LIBPF (ablation builds; never for a reported number)")
+    ap.add_argument("--allow-switches", action="store_true", help="accept PF_* A/B switches in the environment (never for a reported number)")
     args = ap.parse_args()
     if args.also is None:
-        args.also = ["256cube"] if args.workload == "1024sq" else []
+        args.also = ["256cube", "2048sq", "2048sq_f32", "512sq"] if args.workload == "1024sq" else []
     if args.gpus > 1 and "RANK" not in os.environ:
         raise SystemExit(spawn_ranks(args, sys.argv[1:]))
     if args.impl == "reference":

@@ -173,7 +173,8 @@ double pf_fs_kernel_ms(pf_ctx *ctx, int which);
 const char *pf_fs_kernel_name(const pf_ctx *ctx, int which);
 
 /* Timing aid: queues ONLY kernel `which` (0 .. pf_num_fs_kernels()-1) of one Fourier-spectral step on the context's
- * stream (asynchronous, plain launch). A caller brackets a sequence of such calls -- e.g. the same kernel of several
+ * stream (asynchronous; launched as in a step, i.e. with programmatic stream serialization: its table-loading prologue may
+ * overlap the tail of the launch before it, its reads and writes of the fields do not). A caller brackets a sequence of such calls -- e.g. the same kernel of several
  * contexts whose combined state exceeds the L2 -- with its own events. Needs fields (PF_ESTATE otherwise). Afterwards
  * the buffers are no trajectory: pf_step_*, pf_get_fields and pf_free_energy return PF_ESTATE until the next
  * pf_set_fields, further pf_launch_fs_kernel calls are allowed. */

@@ -106,15 +106,21 @@ col2d_kernel(const Col2dParams<T> p)
     // (the twiddle table in shared memory as well was measured slower: 88 KB per CTA needs the next carve-out)
     const CtaSync2 sync;
 
-    // Place in the schedule = blockIdx.x. The grid never exceeds the CTAs that are resident at once, and CTAs are
-    // dispatched in the order of their index, so a consumer item (always in a CTA with an index >= its producer's) cannot
-    // keep its producer off the machine. (A ticket taken with atomicAdd at CTA start instead of blockIdx cost 4.6 us per
-    // launch at 1024^2, profiles/r2_col2d.md.)
+    // Place in the schedule = a ticket, taken in the order in which CTAs START (not blockIdx: CUDA promises neither that
+    // CTAs are dispatched in index order nor that the whole grid is resident at once, e.g. when a second context keeps SMs
+    // busy). Every place lists its C_FWD items -- which wait for nothing -- first, and the consumer of a block sits at a
+    // place >= its producer's; a place is only ever held by a CTA that is already running, so a waiting consumer's
+    // producer is on the machine and finishes: forward progress does not depend on the scheduler.
+    // The counter wraps to zero with the grid's last ticket (atomicInc). It is taken BEFORE griddepcontrol.launch_dependents:
+    // the next launch of this kernel sits two programmatic edges downstream, so none of its CTAs exists before every CTA of
+    // this launch has its ticket. p.ticket == nullptr (PF_COL2D_NOTICKET=1, A/B runs): place = blockIdx.x.
+    __shared__ int s_place;
     for (int i = tid; i < N; i += GT) s_k2[i] = p.ky2[i];
+    if (tid == 0) s_place = p.ticket ? (int)atomicInc(p.ticket, gridDim.x - 1) : (int)blockIdx.x;
     __syncthreads();
-    const int place = blockIdx.x;
+    const int place = s_place;
 
-    grid_dependency_wait();                // everything above touches constant tables only
+    grid_dependency_wait();                // everything above touches constant tables and the ticket only
     grid_dependents_launch();
 
     const T sN = T(1) / T(N);

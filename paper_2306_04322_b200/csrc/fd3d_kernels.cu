@@ -16,6 +16,7 @@
 // The ring of mu is dealt out warp by warp: the two extra rows to warps 0 and 1 (same pair code as the tile rows), the
 // two extra columns to one warp, so no warp runs a pass with two active lanes.
 // Up to four order parameters (126 registers, two CTAs per SM); more run fd_fused3d_kernel.
+#include <atomic>
 #include "pf_kernels.cuh"
 
 namespace pf {
@@ -246,16 +247,23 @@ template <typename T, int NE> static cudaError_t launch_fd3d_march_ne(const FdPa
     constexpr int ES = 4, MS = 3;
     const size_t smem = sizeof(T) * ((size_t)4 * CP + (size_t)(MS + ES * NE) * EP);
     auto kern = fd3d_march_kernel<T, NE>;
-    static int per_sm = 0;                               // resident CTAs per SM of this instantiation
+    // Function attributes and occupancy belong to a DEVICE: a process may hold contexts on several (pf.h), so both are
+    // looked up once per device (index = CUDA device ordinal), not once per process.
+    constexpr int MAXDEV = 64;
+    static std::atomic<int> per_sm_of[MAXDEV];           // resident CTAs per SM of this instantiation; 0 = not yet set up
+    int dev = 0, sms = 148;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) return e;
+    if (dev < 0 || dev >= MAXDEV) return cudaErrorInvalidDevice;
+    cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+    int per_sm = per_sm_of[dev].load(std::memory_order_acquire);
     if (per_sm == 0) {
-        cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-        if (e != cudaSuccess) return e;
+        if ((e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem)) != cudaSuccess) return e;
         int n = 0;
         if ((e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&n, kern, 256, smem)) != cudaSuccess) return e;
         per_sm = n > 0 ? n : 1;
+        per_sm_of[dev].store(per_sm, std::memory_order_release);     // two threads racing here store the same value
     }
-    int dev = 0, sms = 148;
-    if (cudaGetDevice(&dev) == cudaSuccess) cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
     // chunks along z: every chunk re-reads four planes, and the CTAs should fill whole waves. Pick the chunk count with
     // the best (fill of the last wave) x (useful planes / planes read).
     const int tiles = (p.nx / TX) * (p.ny / TY);

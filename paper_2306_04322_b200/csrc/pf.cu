@@ -64,6 +64,7 @@ struct pf_ctx {
     void *carry = nullptr;
     bool carry_valid = false;
     int *c2_sched = nullptr, *c2_sched_init = nullptr, *c2_flags = nullptr;
+    unsigned *c2_ticket = nullptr;       // place counter of the 2D last-axis kernel (nullptr with PF_COL2D_NOTICKET=1)
     int c2_grid = 0, c2_per = 0, c2_grid_init = 0, c2_per_init = 0;
     int sg_cs = 0;                       // > 0: cluster size of the resident small-grid kernel (sgrid_kernels.cu) serving this context
     int carveout = 0;                    // shared-memory carve-out both kernels of a 2D step run with (percent; 0: unset)
@@ -172,7 +173,7 @@ void drop_graph(pf_ctx *c)
 template <typename T> RowParams<T> row_params(pf_ctx *c)
 {
     typedef typename V2<T>::type C;
-    RowParams<T> r;
+    RowParams<T> r{};                    // pdl = 0 unless the caller sets it
     r.zst = (C *)c->zst; r.zg = (C *)c->zg; r.real = (T *)c->real[c->cur];
     r.tw = (const C *)c->tw_m;
     r.zfs = c->B * (c->N / 2); r.rfs = c->B * c->N;   // replicas are further rows of every field
@@ -213,6 +214,7 @@ template <typename T> Col2dParams<T> col2d_params(pf_ctx *c, bool init, bool pdl
     q.sched = init ? c->c2_sched_init : c->c2_sched;
     q.per_cta = init ? c->c2_per_init : c->c2_per;
     q.flags = c->c2_flags;
+    q.ticket = c->c2_ticket;
     q.pdl = pdl;
     q.tw = (const C *)c->tw_y; q.twx = (const C *)c->tw_nx;
     q.kx2 = (const T *)c->kx2; q.ky2 = (const T *)c->ky2;
@@ -251,13 +253,13 @@ template <typename T> cudaError_t mid_forward(pf_ctx *c, const void *zsrc, long 
 // One FS step. 2D: x kernel, y kernel. 3D: x kernel, y-forward, z kernel, y-inverse. All launched with programmatic
 // stream serialization: each kernel's prologue overlaps its predecessor's tail (griddepcontrol in the kernels).
 // events != nullptr: one event after every kernel (profiling; launches are then kept strictly serial).
-// only >= 0: launch just that kernel of the step (timing aid, pf_launch_fs_kernel).
+// only >= 0: launch just that kernel of the step (timing aid, pf_launch_fs_kernel), with the same launch attribute as in a step.
 template <typename T> int fs_one_step(pf_ctx *c, cudaEvent_t *events, int only = -1)
 {
     typedef typename V2<T>::type C;
     const int ny = c->p.n[1], nz = c->p.n[2];
     const long zfs = c->B * (c->N / 2);
-    const bool pdl = events == nullptr && only < 0;
+    const bool pdl = events == nullptr;
     KernelTimer kt(c, events);
     auto want = [&](int k) { return only < 0 || only == k; };
     if (want(0)) {
@@ -398,7 +400,7 @@ template <typename T> int step_fs(pf_ctx *c, int nsteps)
         // Every kernel is launched with programmatic stream serialization, so a kernel's CTAs become resident under its
         // predecessor's last CTAs. Long runs replay a captured graph of kGraphSteps steps (the programmatic edges between
         // ALL its kernels are kept; a graph of one step would serialise at every step boundary: 2.9 us of 52 at 1024^2,
-        // profiles/r2_col2d.md); what is left, and short calls, are plain launches.
+        // DESIGN.md section 2); what is left, and short calls, are plain launches.
         if (!c->fs_graph && c->graph_ok && nsteps >= kGraphSteps) {
             cudaGraph_t g = nullptr;
             const long long before = c->launches;
@@ -563,7 +565,7 @@ const char *pf_strerror(int code)
     case PF_ENOMEM: return "out of device memory";
     case PF_ECUDA: return "CUDA error";
     case PF_ESTATE: return "no fields set";
-    case PF_EUNSUPPORTED: return "unsupported grid size";
+    case PF_EUNSUPPORTED: return "unsupported configuration (grid size, or a feature this kind of context does not have)";
     }
     return "unknown error";
 }
@@ -591,7 +593,7 @@ void pf_destroy(pf_ctx *c)
     for (auto &e : c->pev) if (e) cudaEventDestroy(e);
     void *bufs[] = {c->real[0], c->real[1], c->zst, c->zg, c->s2, c->g2, c->park, c->tw_m, c->tw_y, c->tw_z,
                     c->tw_nx, c->kx2, c->ky2, c->kz2, c->acc, c->queue, c->carry, c->c2_sched, c->c2_sched_init,
-                    c->c2_flags};
+                    c->c2_flags, c->c2_ticket};
     for (void *b : bufs) if (b) cudaFree(b);
     if (c->own_stream) cudaStreamDestroy(c->stream);
     delete c;
@@ -674,6 +676,8 @@ static int create_impl(const pf_params *p, int nbatch, pf_ctx **out)
             (rc = alloc((void **)&c->c2_sched_init, sizeof(int) * sched_init.size())) ||
             (rc = alloc((void **)&c->c2_flags, sizeof(int) * (size_t)nblk_all)))
             return fail(rc);
+        { const char *e = getenv("PF_COL2D_NOTICKET");
+          if (!(e && e[0] == '1') && (rc = alloc((void **)&c->c2_ticket, 64))) return fail(rc); }
         if (cudaMemcpy(c->c2_sched, sched.data(), sizeof(int) * sched.size(), cudaMemcpyHostToDevice) != cudaSuccess ||
             cudaMemcpy(c->c2_sched_init, sched_init.data(), sizeof(int) * sched_init.size(), cudaMemcpyHostToDevice) != cudaSuccess) {
             cudaGetLastError();

@@ -125,6 +125,7 @@ template <typename T> struct Col2dParams {
     int      per_cta;        // items per CTA in sched (padded with -1; at most Col2dShapeInfo::max_items)
     const int *sched;        // [grid][per_cta] items: op | slot << 4 | block << 8
     int     *flags;          // [B*nblk] C_FWD -> C_INV hand-off, zero between launches
+    unsigned *ticket;        // place counter (zero between launches; wraps with the last CTA); nullptr: place = blockIdx.x
     int      pdl;
     const C *tw;             // exp(-2 pi i k / ny)
     const C *twx;            // exp(-2 pi i k / nx), k <= M/2

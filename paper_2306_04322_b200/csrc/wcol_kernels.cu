@@ -214,18 +214,16 @@ template <typename T, int N> static cudaError_t launch_wcol2d_inst(int nslots, c
     const size_t smem = (size_t)N * 4 * sizeof(C) + (size_t)4 * W::THREADS * sizeof(C) + (size_t)W::TT * sizeof(C) +
                         (size_t)N * sizeof(T) + 16;
     auto kern = wcol2d_kernel<T, N>;
-    static int max_ctas = 0;                                // CTAs the device holds at once (per instantiation)
-    if (max_ctas == 0) {
-        cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-        if (e != cudaSuccess) return e;
-        int dev = 0, sms = 0, per_sm = 0;
-        cudaGetDevice(&dev);
-        cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
-        e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kern, W::THREADS, smem);
-        if (e != cudaSuccess) return e;
-        if (per_sm < 1) return cudaErrorLaunchOutOfResources;
-        max_ctas = sms * per_sm;
-    }
+    // attribute and occupancy per launch: both are per device, and this opt-in variant is no hot path
+    cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (e != cudaSuccess) return e;
+    int dev = 0, sms = 0, per_sm = 0;
+    if ((e = cudaGetDevice(&dev)) != cudaSuccess) return e;
+    cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+    e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kern, W::THREADS, smem);
+    if (e != cudaSuccess) return e;
+    if (per_sm < 1) return cudaErrorLaunchOutOfResources;
+    const int max_ctas = sms * per_sm;
     const int grid = nitems < max_ctas ? nitems : max_ctas;
     return launch_pdl(kern, dim3((unsigned)grid), dim3(W::THREADS), smem, s, p.pdl != 0, p, nblk, nitems);
 }

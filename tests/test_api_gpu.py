@@ -124,3 +124,50 @@ def test_single_kernel_launches_leave_no_trajectory():
         ctx.step_fs(2)
         b = ctx.get_fields()
     assert np.array_equal(a[0], b[0]) and np.array_equal(a[1], b[1])
+
+
+def test_two_contexts_on_two_streams_step_concurrently(oracle):
+    # The 2D last-axis kernel hands c^ from one CTA to another through a flag. Its places in the schedule are tickets taken
+    # in the order CTAs start, so the hand-off needs neither the whole grid resident nor index-order dispatch:
+    # two contexts on two non-blocking streams compete for the SMs here, both must finish and both must match the oracle.
+    import torch
+    n, p = (512, 512), 2
+    c, eta, dx = synth.init_b(n, p)
+    streams = [torch.cuda.Stream(), torch.cuda.Stream()]
+    ctxs = [pf.Context(n, n_eta=p, dx=dx, dt=5e-3, stream=s.cuda_stream) for s in streams]
+    try:
+        for ctx in ctxs:
+            ctx.set_fields(c, eta)
+        for _ in range(10):                                  # interleaved single steps and an 8-step graph replay
+            for ctx in ctxs:
+                ctx.step_fs(1)
+        for ctx in ctxs:
+            ctx.step_fs(10)
+        outs = [ctx.get_fields() for ctx in ctxs]
+    finally:
+        for ctx in ctxs:
+            ctx.close()
+    rc, reta = oracle.Model(n=n, n_eta=p, dx=dx, dt=5e-3).step_fs(c, eta, 20)
+    for gc, geta in outs:
+        assert rel_linf([gc, geta], [rc, reta]) < 1e-10
+
+
+def test_fd3d_on_every_visible_device(oracle):
+    # function attributes (the 86 KB dynamic shared memory of the 3D FD kernel) are per device: contexts on every GPU of the
+    # process must step. Needs at least two GPUs; the single-GPU box skips.
+    import torch
+    if torch.cuda.device_count() < 2:
+        pytest.skip("one visible GPU")
+    n, p = (64, 32, 32), 2
+    c, eta, dx = synth.init_b(n, p)
+    rc, reta = oracle.Model(n=n, n_eta=p, dx=dx, dt=1e-3).step_fd(c, eta, 5)
+    try:
+        for d in range(torch.cuda.device_count()):
+            torch.cuda.set_device(d)
+            with pf.Context(n, n_eta=p, dx=dx, dt=1e-3) as ctx:
+                ctx.set_fields(c, eta)
+                ctx.step_fd(5)
+                gc, geta = ctx.get_fields()
+            assert rel_linf([gc, geta], [rc, reta]) < 1e-12, d
+    finally:
+        torch.cuda.set_device(0)
