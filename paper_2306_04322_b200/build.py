@@ -3,6 +3,8 @@
     python -m paper_2306_04322_b200.build [--force]
     PF_EXTRA_NVCC_FLAGS="-DPF_DBG_SKIP_COMPUTE" PF_BUILD_SUFFIX=nocomp python -m paper_2306_04322_b200.build
         -> libpf_nocomp.so beside libpf.so (an ablation / experiment build; load it with PF_LIBPF=<path>, see pf.py)
+    PF_EXTRA_NVCC_FLAGS="-DPF_WCOL" PF_BUILD_SUFFIX=wcol ...   adds wcol_kernels.cu (persistent pipelined strided kernel, selected at
+        run time with PF_WCOL=1); PF_EXTRA_NVCC_FLAGS="-DPF_WFFT" the warp-tile FFT. Neither is part of the default library.
 
 The translation units are compiled in parallel and linked into
 paper_2306_04322_b200/libpf.so (static cudart; no torch, no other dependency).
@@ -20,8 +22,10 @@ CSRC = os.path.join(HERE, "csrc")
 SUFFIX = os.environ.get("PF_BUILD_SUFFIX", "")
 OBJ = os.path.join(HERE, "csrc", "build" + ("_" + SUFFIX if SUFFIX else ""))
 SO = os.path.join(HERE, "libpf" + ("_" + SUFFIX if SUFFIX else "") + ".so")
-UNITS = ["row_kernels", "col_kernels", "col2d_kernels", "wcol_kernels", "fd_kernels", "fd2d_kernels", "fd3d_kernels", "sgrid_kernels", "static_energy", "pf"]
+UNITS = ["row_kernels", "col_kernels", "col2d_kernels", "fd_kernels", "fd2d_kernels", "fd3d_kernels", "sgrid_kernels", "static_energy", "pf"]
 HEADERS = sorted(glob.glob(os.path.join(CSRC, "*.cuh"))) + [os.path.join(os.path.dirname(HERE), "include", "pf.h")]
+if "-DPF_WCOL" in os.environ.get("PF_EXTRA_NVCC_FLAGS", "").split():       # opt-in variant (profiles/r2_col_variants.md)
+    UNITS.insert(3, "wcol_kernels")
 NVCC_FLAGS = ["-std=c++17", "-O3", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo",
               "-Xcompiler", "-fPIC", "-Xptxas", "-v"] + os.environ.get("PF_EXTRA_NVCC_FLAGS", "").split()
 

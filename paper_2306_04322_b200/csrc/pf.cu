@@ -46,7 +46,7 @@ struct pf_ctx {
     cudaStream_t stream = nullptr;
     bool own_stream = false;
     bool graph_ok = true;
-    bool use_wcol = false;              // PF_WCOL=1 in the environment: the persistent pipelined strided kernel (A/B runs, profiles/)
+    bool use_wcol = false;              // -DPF_WCOL builds with PF_WCOL=1 in the environment: the persistent pipelined strided kernel (A/B runs, profiles/)
     void *real[2] = {nullptr, nullptr};
     int cur = 0;
     void *zst = nullptr, *zg = nullptr, *s2 = nullptr, *g2 = nullptr, *park = nullptr;
@@ -277,8 +277,11 @@ template <typename T> int fs_one_step(pf_ctx *c, cudaEvent_t *events, int only =
             q.in0 = zst; q.in1 = (const C *)c->zg; q.out = zst; q.in_fs = q.out_fs = zfs;
             q.has_c = 1; q.pdl = pdl;
             cudaError_t e = cudaErrorNotSupported;
+#ifdef PF_WCOL
             if (c->use_wcol) e = launch_wcol2d<T>(ny, c->F, q, c->stream);
-            else if (!c->legacy_col2d) e = launch_col2d<T>(ny, col2d_params<T>(c, false, pdl), c->c2_grid, c->stream);
+            else
+#endif
+            if (!c->legacy_col2d) e = launch_col2d<T>(ny, col2d_params<T>(c, false, pdl), c->c2_grid, c->stream);
             if (e == cudaErrorNotSupported) e = launch_col<T>(COL_2D_LAST, ny, c->F, 1, q, c->stream);
             PF_CK(c, e); ++c->launches;
         }
@@ -622,7 +625,9 @@ static int create_impl(const pf_params *p, int nbatch, pf_ctx **out)
     c->p = *p;
     c->B = nbatch;
     c->device = dev;
+#ifdef PF_WCOL                       // the measured-slower persistent strided kernel is compiled into ablation builds only
     { const char *e = getenv("PF_WCOL"); c->use_wcol = (e && e[0] == '1' && nbatch == 1); }
+#endif
     { const char *e = getenv("PF_COL2D_LEGACY"); c->legacy_col2d = (e && e[0] == '1' && nbatch == 1); }
     { const char *e = getenv("PF_COL3D_PARK"); c->park3d = (e && e[0] == '1'); }
     { const char *e = getenv("PF_FD2D_LEGACY"); c->legacy_fd2d = (e && e[0] == '1'); }

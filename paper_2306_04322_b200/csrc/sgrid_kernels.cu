@@ -16,7 +16,9 @@
 // touches global memory between the first and the last step. c^ is carried, as in Algorithm 1: the warp that updates a
 // pair of Cahn-Hilliard columns keeps their spectrum in its CTA's shared memory (filled once per launch from the z-form
 // of c), so a Cahn-Hilliard column costs two transforms per step like an Allen-Cahn column.
-// Square grids 32^2 ... 256^2, both precisions; the host picks the cluster size (1..16) from the state size.
+// Square grids 32^2 ... 256^2, both precisions, as far as the state plus the carried c^ fits the shared memory of 16 CTAs:
+// every field count up to 128^2 and at 256^2 in fp32; 256^2 in fp64 only with few fields (c + 2 eta no longer fits since c^ is
+// carried: sgrid_plan returns 0 and the context stays on the two-kernel path). The host picks the cluster size (1..16).
 #include <cooperative_groups.h>
 
 #include "pf_kernels.cuh"
