@@ -621,7 +621,14 @@ def small_grid_measurements(env):
 
     out = {"workload": "2D 64x64, c + 2 eta, fp64, seeded noise, dt = 0.05 (configs[0])",
            "single_simulation_cluster_resident": single(True), "single_simulation_two_kernel_path": single(False),
-           "single_256sq_c_4eta_two_kernel_path": single(True, (256, 256), 4)}
+           "single_256sq_c_4eta_two_kernel_path": single(True, (256, 256), 4),
+           "single_128sq_c_4eta_two_kernel_path": single(True, (128, 128), 4)}
+    # the paper's small 3D grids (Table 2; 16^3 and 32^3 "increase significantly"): one
+    # simulation, c + 2 eta, fp64, four launches per step replayed as an 8-step graph -- launch-latency bound, reported as is
+    for m in (16, 32, 64):
+        r = single(True, (m, m, m), 2)
+        r["frac_of_hbm_roofline_on_survey_8d_bytes"] = (3 * (2 * m ** 3 * 8 + 11 * (m // 2 + 1) * m * m * 16)) * r["value"] / 1e9 / peaks()[0]
+        out[f"single_{m}cube_c_2eta"] = r
     B = 64
     inits = [synth.init_a(n, p, seed=100 + b) for b in range(B)]
     c0, e0 = np.stack([c for c, _ in inits]), np.stack([e for _, e in inits])

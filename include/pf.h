@@ -168,6 +168,13 @@ int    pf_set_profiling(pf_ctx *ctx, int on);
  * best of three timed launches. Diagnostic for the roofline notes (the Fourier-spectral kernels are
  * bound by fp64 issue and shared memory as much as by HBM). Synchronises the device. PF_EINVAL / PF_ECUDA on failure. */
 int    pf_fp64_fma_peak(double *tflops);
+/* Measured read rate of distributed shared memory on the current device: bytes per SM clock per SM that the CTAs of a
+ * thread-block cluster of cluster_size CTAs (1, 2, 4, 8, 16) load from each other's shared memory with 16-byte loads
+ * (remote != 0), or from their own through the same address path (remote == 0); one CTA per SM, the slowest CTA counts.
+ * Diagnostic for DESIGN.md section 6 (why the 3D y/z passes are not merged inside a cluster; where the cluster-resident
+ * small-grid kernel stops paying off). Allocates two small device buffers, synchronises the device.
+ * PF_EINVAL: bad arguments; PF_EUNSUPPORTED: the device cannot run clusters of that size; PF_ENOMEM / PF_ECUDA. */
+int    pf_dsmem_read_rate(int cluster_size, int remote, double *bytes_per_clk_per_sm);
 int    pf_num_fs_kernels(const pf_ctx *ctx);
 double pf_fs_kernel_ms(pf_ctx *ctx, int which);
 const char *pf_fs_kernel_name(const pf_ctx *ctx, int which);

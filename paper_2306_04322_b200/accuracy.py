@@ -44,6 +44,35 @@ def advance(pf, n, p, dx, dt, t_span, c, eta, method="fs", k2_kind=0):
         return out_c, out_eta, steps, time.perf_counter() - t0
 
 
+def restrict(u, r, how):
+    """A periodic fine-grid field u[..., ny, nx] on the grid that keeps every r-th point (the grids nest). Harness code:
+    PAPER.md:65 does not say how the t = 1 field reaches the coarse grids.
+      sample    point sampling u[::r, ::r] (aliases what the coarse grid cannot carry);
+      spectral  Fourier truncation: the modes |k| < n/2 of the fine field, evaluated on the coarse points;
+      average   mean over the coarse cell centred on each coarse point (trapezoid weights, periodic)."""
+    if r == 1 or how == "sample":
+        return np.ascontiguousarray(u[..., ::r, ::r])
+    ny, nx = u.shape[-2:]
+    my, mx = ny // r, nx // r
+    if how == "spectral":
+        U = np.fft.fft2(u)
+        ky, kx = np.fft.fftfreq(ny, 1.0 / ny), np.fft.fftfreq(nx, 1.0 / nx)
+        keep = (np.abs(ky)[:, None] < my / 2) & (np.abs(kx)[None, :] < mx / 2)
+        iy, ix = np.nonzero(np.abs(ky) < my / 2)[0], np.nonzero(np.abs(kx) < mx / 2)[0]
+        V = np.zeros(u.shape[:-2] + (my, mx), dtype=complex)
+        V[..., (ky[iy].astype(int) % my)[:, None], (kx[ix].astype(int) % mx)[None, :]] = (U * keep)[..., iy[:, None], ix[None, :]]
+        return np.ascontiguousarray(np.fft.ifft2(V).real / (r * r))
+    if how == "average":
+        w = np.ones(r + 1)
+        w[0] = w[-1] = 0.5
+        w /= w.sum()
+        out = u
+        for axis in (-2, -1):
+            out = sum(wk * np.roll(out, r // 2 - k, axis=axis) for k, wk in enumerate(w))
+        return np.ascontiguousarray(out[..., ::r, ::r])
+    raise ValueError(how)
+
+
 def main():
     from . import pf, synth
 
@@ -56,6 +85,9 @@ def main():
     ap.add_argument("--pre", default="fs", choices=["fs", "fd"],
                     help="pre-evolution t = 0 -> 1 on the reference grid: the FS step at --ref-dt (stand-in) or, as the paper "
                          "describes it (PAPER.md:65), explicit FD at 0.75 x its stability limit on that grid (sensitivity run)")
+    ap.add_argument("--restrict", nargs="+", default=["sample"], choices=["sample", "spectral", "average"],
+                    help="how the t = 1 field of the reference grid is put on the coarse grids (PAPER.md:65 is silent); the "
+                         "coarse results are always compared with the reference at the coarse points")
     ap.add_argument("--out", default=None)
     a = ap.parse_args()
     p, length = 4, 200.0
@@ -76,10 +108,12 @@ def main():
           f"(finite: {bool(np.isfinite(cr).all())})", flush=True)
     rows = []
     print(f"{'grid':>6} {'method':>14} {'dt':>10} {'steps':>9} {'seconds':>8} {'E_c %':>11} {'E_eta %':>11}")
-    for n in a.grids:
+    for how, n in [(h, g) for h in a.restrict for g in a.grids]:
+        if len(a.restrict) > 1 or how != "sample":
+            print(f"# t = 1 field restricted to {n}^2 by: {how}", flush=True)
         r = nr // n
         dx = length / n
-        ci, ei = np.ascontiguousarray(c1[::r, ::r]), np.ascontiguousarray(eta1[:, ::r, ::r])
+        ci, ei = restrict(c1, r, how), restrict(eta1, r, how)
         rc, rs = cr[::r, ::r], er.sum(0)[::r, ::r]
         k2max = 8.0 / dx ** 2
         dt_fd = min(0.75 * 2.0 / (M * k2max * (2 * rho2 + kc * k2max)), 2e-3)
@@ -92,7 +126,7 @@ def main():
                 continue
             gc, ge, steps, sec = advance(pf, n, p, dx, dt, a.t_end - 1.0, ci, ei, method, kind)
             fin = bool(np.isfinite(gc).all() and np.isfinite(ge).all())
-            row = {"grid": n, "method": name, "dt": dt, "steps": steps, "seconds": sec, "finite": fin,
+            row = {"grid": n, "restrict": how, "method": name, "dt": dt, "steps": steps, "seconds": sec, "finite": fin,
                    "E_c_percent": eq22_percent(gc, rc) if fin else None,
                    "E_eta_percent": eq22_percent(ge.sum(0), rs) if fin else None}
             rows.append(row)

@@ -22,7 +22,7 @@ CSRC = os.path.join(HERE, "csrc")
 SUFFIX = os.environ.get("PF_BUILD_SUFFIX", "")
 OBJ = os.path.join(HERE, "csrc", "build" + ("_" + SUFFIX if SUFFIX else ""))
 SO = os.path.join(HERE, "libpf" + ("_" + SUFFIX if SUFFIX else "") + ".so")
-UNITS = ["row_kernels", "col_kernels", "col2d_kernels", "fd_kernels", "fd2d_kernels", "fd3d_kernels", "sgrid_kernels", "static_energy", "pf"]
+UNITS = ["row_kernels", "col_kernels", "col2d_kernels", "fd_kernels", "fd2d_kernels", "fd3d_kernels", "sgrid_kernels", "static_energy", "dsmem_probe", "pf"]
 HEADERS = sorted(glob.glob(os.path.join(CSRC, "*.cuh"))) + [os.path.join(os.path.dirname(HERE), "include", "pf.h")]
 if "-DPF_WCOL" in os.environ.get("PF_EXTRA_NVCC_FLAGS", "").split():       # opt-in variant (profiles/r2_col_variants.md)
     UNITS.insert(3, "wcol_kernels")

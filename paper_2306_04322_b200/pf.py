@@ -20,7 +20,7 @@ PF_HOST, PF_DEVICE = 0, 1
 PF_OK, PF_EINVAL, PF_ENOMEM, PF_ECUDA, PF_ESTATE, PF_EUNSUPPORTED = 0, -1, -2, -3, -4, -5
 
 EXPORTS = ["pf_create", "pf_create_batch", "pf_batch_size", "pf_set_fields", "pf_step_fs", "pf_step_fd", "pf_get_fields", "pf_free_energy",
-           "pf_free_energy_static", "pf_set_dt", "pf_launch_count", "pf_fp64_fma_peak", "pf_set_profiling", "pf_num_fs_kernels", "pf_fs_kernel_ms", "pf_launch_fs_kernel",
+           "pf_free_energy_static", "pf_set_dt", "pf_launch_count", "pf_fp64_fma_peak", "pf_dsmem_read_rate", "pf_set_profiling", "pf_num_fs_kernels", "pf_fs_kernel_ms", "pf_launch_fs_kernel",
            "pf_fs_kernel_name", "pf_strerror", "pf_last_cuda_error", "pf_destroy"]
 
 
@@ -78,6 +78,8 @@ def lib() -> ctypes.CDLL:
         L.pf_launch_count.argtypes = [vp]
         L.pf_fp64_fma_peak.restype = ctypes.c_int
         L.pf_fp64_fma_peak.argtypes = [ctypes.POINTER(ctypes.c_double)]
+        L.pf_dsmem_read_rate.restype = ctypes.c_int
+        L.pf_dsmem_read_rate.argtypes = [ctypes.c_int, ctypes.c_int, ctypes.POINTER(ctypes.c_double)]
         L.pf_set_profiling.restype = ctypes.c_int
         L.pf_set_profiling.argtypes = [vp, ctypes.c_int]
         L.pf_num_fs_kernels.restype = ctypes.c_int
@@ -144,6 +146,15 @@ def free_energy_static(c, eta, n, **kw):
     if rc != PF_OK:
         raise PfError(rc, "pf_free_energy_static", lib().pf_strerror(rc).decode())
     return np.array(out[:], dtype=np.float64)
+
+
+def dsmem_read_rate(cluster_size: int, remote: bool = True) -> float:
+    """Measured distributed-shared-memory read rate, bytes per SM clock per SM (pf_dsmem_read_rate)."""
+    out = ctypes.c_double()
+    rc = lib().pf_dsmem_read_rate(int(cluster_size), int(bool(remote)), ctypes.byref(out))
+    if rc != PF_OK:
+        raise PfError(rc, "pf_dsmem_read_rate", lib().pf_strerror(rc).decode())
+    return float(out.value)
 
 
 class Context:

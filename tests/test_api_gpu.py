@@ -171,3 +171,13 @@ def test_fd3d_on_every_visible_device(oracle):
             assert rel_linf([gc, geta], [rc, reta]) < 1e-12, d
     finally:
         torch.cuda.set_device(0)
+
+
+def test_dsmem_read_rate_probe():
+    # diagnostic of DESIGN.md section 6: own shared memory is at least as fast as a neighbour's; sizes that are no power of
+    # two are refused
+    own = pf.dsmem_read_rate(4, remote=False)
+    rem = pf.dsmem_read_rate(4, remote=True)
+    assert 1.0 < rem <= own * 1.05 and own < 300.0           # bytes per clock per SM: 128 is the shared-memory pipe's width
+    with pytest.raises(pf.PfError):
+        pf.dsmem_read_rate(3)
