@@ -651,6 +651,25 @@ def small_grid_measurements(env):
     out["batch_of_64_replicas"] = {"one_context_replica_steps_per_s": 1e3 * B / msb, "us_per_step_of_all_replicas": 1e3 * msb,
                                    "loop_over_64_contexts_replica_steps_per_s": 1e3 * B / msl, "ratio": msl / msb,
                                    "note": "pf_create_batch(nbatch=64) + pf_step_fs(K) against pf_step_fs(1) on 64 contexts in turn"}
+    # 3D: 64 replicas of 32^3 (c + 2 eta) in one context against a loop over 64 contexts
+    n3 = (32, 32, 32)
+    inits = [synth.init_a(n3, p, seed=200 + b) for b in range(B)]
+    c0, e0 = np.stack([c for c, _ in inits]), np.stack([e for _, e in inits])
+    with pf.Context(n3, n_eta=p, dx=1.0, dt=0.05, nbatch=B, stream=stream.cuda_stream) as cx:
+        cx.set_fields(c0, e0)
+        cx.step_fs(16)
+        msb = stats([timed(lambda: cx.step_fs(200)) for _ in range(5)])["median"] / 200
+    cxs = [pf.Context(n3, n_eta=p, dx=1.0, dt=0.05, stream=stream.cuda_stream) for _ in range(B)]
+    for b, cx in enumerate(cxs):
+        cx.set_fields(c0[b], e0[b])
+        cx.step_fs(4)
+    msl = stats([timed(loop) for _ in range(3)])["median"] / 20
+    for cx in cxs:
+        cx.close()
+    out["batch_of_64_replicas_32cube"] = {"one_context_replica_steps_per_s": 1e3 * B / msb, "us_per_step_of_all_replicas": 1e3 * msb,
+                                          "loop_over_64_contexts_replica_steps_per_s": 1e3 * B / msl, "ratio": msl / msb,
+                                          "frac_of_hbm_roofline_on_survey_8d_bytes": B * 3 * (2 * 32 ** 3 * 8 + 11 * 17 * 32 * 32 * 16) / (msb * 1e-3) / 1e9 / peaks()[0],
+                                          "note": "pf_create_batch(nbatch=64) on 32^3 + pf_step_fs(200) against pf_step_fs(1) on 64 contexts in turn"}
     return out
 
 

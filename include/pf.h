@@ -68,14 +68,15 @@ int pf_create(const pf_params *p, pf_ctx **out);
 
 /* Batched small grids (the paper reports that small grids leave the GPU idle: PAPER.md:265, 128^2 "less than 3.8 grid
  * points per CUDA core", 16^3 and 32^3). Creates ONE context that advances nbatch independent replicas of
- * the 2D problem described by p -- same grid, coefficients and dt, different fields -- with the same kernels and the same
- * number of launches per step as a single simulation: the replicas are further rows of the x kernel and further column
- * blocks of the last-axis kernel. Field arrays of such a context are replica-major:
- *     c: [nbatch][ny][nx],   eta: [nbatch][n_eta][ny][nx]
+ * the 2D or 3D problem described by p -- same grid, coefficients and dt, different fields -- with the same kernels and the
+ * same number of launches per Fourier-spectral step as a single simulation: the replicas are further rows of the x kernel,
+ * further planes of the 3D y kernels and further column blocks of the last-axis kernel. Field arrays of such a context are
+ * replica-major:
+ *     c: [nbatch][nz][ny][nx],   eta: [nbatch][n_eta][nz][ny][nx]
  * and every replica evolves exactly as it would in its own context (tests compare each with the oracle).
- * pf_step_fs, pf_step_fd, pf_set_fields, pf_get_fields and pf_set_dt work as for a single simulation;
- * pf_free_energy returns PF_EUNSUPPORTED (read the fields out instead).
- * PF_EINVAL: nbatch outside 1..4096 (and everything pf_create rejects); PF_EUNSUPPORTED: ndim == 3 with nbatch > 1.
+ * pf_step_fs, pf_step_fd, pf_set_fields, pf_get_fields and pf_set_dt work as for a single simulation (pf_step_fd of a 3D
+ * batch issues one launch per replica and step); pf_free_energy returns PF_EUNSUPPORTED (read the fields out instead).
+ * PF_EINVAL: nbatch outside 1..4096 (and everything pf_create rejects); PF_EUNSUPPORTED: ndim == 3 with nz * nbatch > 65535.
  * nbatch == 1 is pf_create. */
 int pf_create_batch(const pf_params *p, int nbatch, pf_ctx **out);
 

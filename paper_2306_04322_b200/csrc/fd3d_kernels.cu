@@ -87,7 +87,7 @@ __global__ void __launch_bounds__(256, 2) fd3d_march_kernel(const FdParams<T> p,
     auto load_e = [&](int m, int slot) {
 #pragma unroll
         for (int f = 0; f < NE; ++f) {
-            const T *src = p.eta + (long)f * p.N + (long)((z0 + m) & mz) * plane;
+            const T *src = p.eta + (long)f * p.fs + (long)((z0 + m) & mz) * plane;
             T *dst = se + (f * ES + slot) * EP;
 #pragma unroll
             for (int i = 0; i < NEC; ++i)
@@ -176,7 +176,7 @@ __global__ void __launch_bounds__(256, 2) fd3d_march_kernel(const FdParams<T> p,
             P2 en;
             en.x = e0[f].x - p.m.dtL * (dfdeta(p.m, ck.x, e0[f].x, s0) - p.m.kappa_eta * le.x);
             en.y = e0[f].y - p.m.dtL * (dfdeta(p.m, ck.y, e0[f].y, s1) - p.m.kappa_eta * le.y);
-            *reinterpret_cast<P2 *>(p.eta_new + (long)f * p.N + g) = en;
+            *reinterpret_cast<P2 *>(p.eta_new + (long)f * p.fs + g) = en;
         }
     };
 

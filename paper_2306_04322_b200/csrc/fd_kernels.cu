@@ -148,7 +148,7 @@ __global__ void __launch_bounds__(TX * TY) fd_fused3d_kernel(const FdParams<T> p
     };
     auto load_e = [&](int m) {
         for (int k = 0; k < NE; ++k) {
-            const T *src = p.eta + (long)k * p.N + (long)((z0 + m) & mz) * plane;
+            const T *src = p.eta + (long)k * p.fs + (long)((z0 + m) & mz) * plane;
             T *dst = se + (k * 4 + ((m + 4) & 3)) * EP;
             for (int ly = ty; ly < EH; ly += TY) {
                 const T *row = src + (long)((y0 + ly - 1) & my) * p.nx;
@@ -215,7 +215,7 @@ __global__ void __launch_bounds__(TX * TY) fd_fused3d_kernel(const FdParams<T> p
             const T ezp = se[(f * 4 + ((k + 5) & 3)) * EP + e0], ezm = se[(f * 4 + ((k + 3) & 3)) * EP + e0];
             const T le = p.rdx2[0] * (e[1] + e[-1] - T(2) * e[0]) + p.rdx2[1] * (e[EW] + e[-EW] - T(2) * e[0])
                        + p.rdx2[2] * (ezp + ezm - T(2) * e[0]);
-            p.eta_new[(long)f * p.N + g] = e[0] - p.m.dtL * (dfdeta(p.m, c, e[0], s2) - p.m.kappa_eta * le);
+            p.eta_new[(long)f * p.fs + g] = e[0] - p.m.dtL * (dfdeta(p.m, c, e[0], s2) - p.m.kappa_eta * le);
         }
         s3 = s3p;
     }

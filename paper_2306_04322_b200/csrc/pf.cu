@@ -39,7 +39,7 @@ struct pf_ctx {
     pf_params p;
     int F = 1, M = 0, P2 = 0;
     long N = 0;                          // grid points of ONE replica
-    int B = 1;                           // replicas advanced together (pf_create_batch; 2D only)
+    int B = 1;                           // replicas advanced together (pf_create_batch): further rows / planes / column blocks of the same launches
     int c2_nblk = 0;                     // column blocks per replica of the 2D last-axis kernel
     size_t w = 8;
     int device = 0;                      // the CUDA device the context was created on (every call checks it is current)
@@ -247,7 +247,7 @@ template <typename T> cudaError_t mid_forward(pf_ctx *c, const void *zsrc, long 
     q.tw = (const C *)c->tw_y;
     q.pdl = pdl;
     ++c->launches;
-    return launch_col<T>(COL_3D_MIDFWD, ny, nslots, nz, q, c->stream);
+    return launch_col<T>(COL_3D_MIDFWD, ny, nslots, nz * c->B, q, c->stream);    // replicas are further planes
 }
 
 // One FS step. 2D: x kernel, y kernel. 3D: x kernel, y-forward, z kernel, y-inverse. All launched with programmatic
@@ -287,7 +287,8 @@ template <typename T> int fs_one_step(pf_ctx *c, cudaEvent_t *events, int only =
         }
         kt.mark("col_y_fft_update_ifft");
     } else {
-        const long s2fs = (long)nz * ny * c->P2;
+        const long s2rs = (long)nz * ny * c->P2;               // one replica of one field
+        const long s2fs = s2rs * c->B;
         C *s2 = (C *)c->s2;
         if (want(1)) PF_CK(c, mid_forward<T>(c, zst, zfs, s2, s2fs, c->F, true, pdl));
         kt.mark("col_y_fwd");
@@ -296,8 +297,9 @@ template <typename T> int fs_one_step(pf_ctx *c, cudaEvent_t *events, int only =
             q.tw = (const C *)c->tw_z;
             q.in_rs = q.out_rs = (long)ny * c->P2; q.ncols = ny * c->P2;
             q.in0 = s2; q.in1 = (const C *)c->g2; q.out = s2; q.in_fs = q.out_fs = s2fs;
+            q.in_bs = q.out_bs = s2rs;                         // blockIdx.y = replica
             q.has_c = c->park3d ? 1 : 2; q.pdl = pdl;          // 2: c^ carried in `park` (filled by to_spectral)
-            PF_CK(c, launch_col<T>(COL_3D_LAST, nz, c->F, 1, q, c->stream)); ++c->launches;
+            PF_CK(c, launch_col<T>(COL_3D_LAST, nz, c->F, c->B, q, c->stream)); ++c->launches;
         }
         kt.mark("col_z_fft_update_ifft");
         if (want(3)) {
@@ -306,7 +308,7 @@ template <typename T> int fs_one_step(pf_ctx *c, cudaEvent_t *events, int only =
             v.in0 = s2; v.in_fs = s2fs; v.in_rs = c->P2; v.in_bs = (long)ny * c->P2;
             v.out = zst; v.out_fs = zfs; v.out_rs = c->M; v.out_bs = (long)ny * c->M;
             v.pdl = pdl;
-            PF_CK(c, launch_col<T>(COL_3D_MIDINV, ny, c->F, nz, v, c->stream)); ++c->launches;
+            PF_CK(c, launch_col<T>(COL_3D_MIDINV, ny, c->F, nz * c->B, v, c->stream)); ++c->launches;
         }
         kt.mark("col_y_inv");
     }
@@ -336,9 +338,10 @@ template <typename T> int to_spectral(pf_ctx *c, bool need_carry = true)
             q.tw = (const C *)c->tw_z;
             q.in_rs = q.out_rs = (long)ny * c->P2; q.ncols = ny * c->P2;
             q.in0 = (const C *)c->s2; q.in1 = (const C *)c->g2; q.out = (C *)c->s2;
-            q.in_fs = q.out_fs = (long)nz * ny * c->P2;
+            q.in_fs = q.out_fs = (long)nz * ny * c->P2 * c->B;
+            q.in_bs = q.out_bs = (long)nz * ny * c->P2;
             q.has_c = 3; q.pdl = 0;
-            PF_CK(c, launch_col<T>(COL_3D_LAST, nz, 1, 1, q, c->stream)); ++c->launches;
+            PF_CK(c, launch_col<T>(COL_3D_LAST, nz, 1, c->B, q, c->stream)); ++c->launches;
         }
         c->s2c_valid = true;
     }
@@ -451,10 +454,15 @@ template <typename T> int step_fd(pf_ctx *c, int nsteps)
             PF_CK(c, e);
             c->launches += 1;
         } else {
-            cudaError_t e = c->legacy_fd3d ? cudaErrorNotSupported : launch_fd3d_march<T>(f, c->stream);
-            if (e == cudaErrorNotSupported) e = launch_fd_fused3d<T>(f, c->stream);
-            PF_CK(c, e);
-            c->launches += 1;
+            for (int b = 0; b < c->B; ++b) {             // 3D: one launch per replica (the z chunks take blockIdx.z)
+                FdParams<T> g = f;
+                g.nbatch = 1;
+                g.c += (long)b * c->N; g.eta += (long)b * c->N; g.c_new += (long)b * c->N; g.eta_new += (long)b * c->N;
+                cudaError_t e = c->legacy_fd3d ? cudaErrorNotSupported : launch_fd3d_march<T>(g, c->stream);
+                if (e == cudaErrorNotSupported) e = launch_fd_fused3d<T>(g, c->stream);
+                PF_CK(c, e);
+                c->launches += 1;
+            }
         }
         c->cur ^= 1;
     }
@@ -606,7 +614,6 @@ static int create_impl(const pf_params *p, int nbatch, pf_ctx **out)
 {
     if (!p || !out) return PF_EINVAL;
     if (nbatch < 1 || nbatch > 4096) return PF_EINVAL;
-    if (nbatch > 1 && p->ndim != 2) return PF_EUNSUPPORTED;
     if (p->ndim != 2 && p->ndim != 3) return PF_EINVAL;
     if (p->n_eta < 0 || p->n_eta > 8) return PF_EINVAL;
     if (!(p->dt > 0.0)) return PF_EINVAL;
@@ -615,6 +622,7 @@ static int create_impl(const pf_params *p, int nbatch, pf_ctx **out)
     for (int d = 0; d < p->ndim; ++d) if (!(p->dx[d] > 0.0)) return PF_EINVAL;
     for (int d = 0; d < p->ndim; ++d) if (!pow2_in_range(p->n[d])) return PF_EUNSUPPORTED;
     if (p->ndim == 2 && p->n[2] != 1) return PF_EUNSUPPORTED;
+    if (p->ndim == 3 && (long)p->n[2] * nbatch > 65535) return PF_EUNSUPPORTED;      // planes of all replicas = blockIdx.y of the y kernels
 
     int ndev = 0, dev = 0;
     if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev <= 0) { cudaGetLastError(); return PF_ECUDA; }
@@ -661,7 +669,7 @@ static int create_impl(const pf_params *p, int nbatch, pf_ctx **out)
         (rc = alloc(&c->park, (size_t)(c->P2 + 16) * c->p.n[1] * c->p.n[2] * 2 * c->w * c->B)))
         return fail(rc);
     if (p->ndim == 3) {
-        const size_t pb = (size_t)c->p.n[2] * c->p.n[1] * c->P2 * 2 * c->w;
+        const size_t pb = (size_t)c->p.n[2] * c->p.n[1] * c->P2 * 2 * c->w * c->B;
         if ((rc = alloc(&c->s2, pb * c->F)) || (rc = alloc(&c->g2, pb))) return fail(rc);
     }
     rc = (p->precision == PF_F64) ? upload_tables<double>(c) : upload_tables<float>(c);

@@ -54,13 +54,14 @@ def test_argument_validation_without_gpu(libpf):
                       (dict(n=(64, 64), k2_kind=3), libpf.PF_EINVAL), (dict(n=(64, 64), precision=7), libpf.PF_EINVAL)]:
         q = libpf.make_params(**bad)
         assert L.pf_create(ctypes.byref(q), ctypes.byref(h)) == code, bad
-    # batched contexts (pf_create_batch): replica count 1..4096, 2D only; checked before any device is touched
+    # batched contexts (pf_create_batch): replica count 1..4096, in 3D at most 65535 planes over all replicas; checked before
+    # any device is touched
     q = libpf.make_params((64, 64), n_eta=2)
     assert L.pf_create_batch(ctypes.byref(q), 0, ctypes.byref(h)) == libpf.PF_EINVAL
     assert L.pf_create_batch(ctypes.byref(q), 5000, ctypes.byref(h)) == libpf.PF_EINVAL
     assert L.pf_create_batch(None, 4, ctypes.byref(h)) == libpf.PF_EINVAL
     q3 = libpf.make_params((32, 32, 32), n_eta=2)
-    assert L.pf_create_batch(ctypes.byref(q3), 4, ctypes.byref(h)) == libpf.PF_EUNSUPPORTED
+    assert L.pf_create_batch(ctypes.byref(q3), 4096, ctypes.byref(h)) == libpf.PF_EUNSUPPORTED
     assert L.pf_batch_size(None) == 0
     assert L.pf_step_fs(None, 1) == libpf.PF_EINVAL
     assert L.pf_launch_count(None) == 0

@@ -93,7 +93,58 @@ def test_batch_of_one_equals_single_context_bitwise():
     assert np.array_equal(ac, bc[0]) and np.array_equal(ae, be[0])
 
 
-def test_batch_rejects_3d():
+def test_batch_rejects_more_planes_than_a_grid_dimension_holds():
+    # 3D: the planes of all replicas are blockIdx.y of the y kernels (at most 65535)
     h = ctypes.c_void_p()
     q = pf.make_params((32, 32, 32), n_eta=2)
-    assert pf.lib().pf_create_batch(ctypes.byref(q), 2, ctypes.byref(h)) == pf.PF_EUNSUPPORTED
+    assert pf.lib().pf_create_batch(ctypes.byref(q), 4096, ctypes.byref(h)) == pf.PF_EUNSUPPORTED
+
+
+@pytest.mark.parametrize("n,p,B,steps,precision,tol", [((16, 16, 16), 2, 5, 40, "f64", 1e-10), ((32, 32, 32), 2, 4, 30, "f64", 1e-10),
+                                                       ((64, 32, 16), 4, 3, 20, "f64", 1e-10), ((32, 16, 64), 0, 6, 20, "f64", 1e-10),
+                                                       ((32, 32, 32), 2, 3, 30, "f32", 1e-4), ((64, 64, 64), 1, 2, 10, "f64", 1e-10)])
+def test_batch_3d_fs(oracle, n, p, B, steps, precision, tol):
+    # 3D batches (the paper's small 3D grids, Table 2 / PAPER.md:267): replicas are further planes of the x and y kernels and
+    # further column blocks (blockIdx.y) of the z kernel with its carried c^; anisotropic shapes so no stride can be swapped
+    c, eta, dx = synth.init_b(n, p)
+    rng = np.random.default_rng(11)
+    c0 = np.stack([c + 0.02 * rng.standard_normal(c.shape) for _ in range(B)])
+    e0 = np.stack([eta + 0.01 * rng.standard_normal(eta.shape) for _ in range(B)])
+    with pf.Context(n, n_eta=p, dx=dx, dt=5e-3, precision=precision, nbatch=B) as ctx:
+        ctx.set_fields(c0, e0)
+        l0 = ctx.launch_count()
+        ctx.step_fs(steps // 2)
+        mid = ctx.get_fields()                       # read-out in the middle: the carried spectra survive it
+        ctx.step_fs(steps - steps // 2)
+        launches = ctx.launch_count() - l0
+        gc, ge = ctx.get_fields()
+    assert gc.shape == (B,) + tuple(reversed(n)) and ge.shape == (B, p) + tuple(reversed(n)) and mid[0].shape == gc.shape
+    assert launches <= 4 * steps + 6                 # the launches of ONE simulation
+    m = oracle.Model(n=n, n_eta=p, dx=dx, dt=5e-3)
+    for b in range(B):
+        ci, ei = c0[b], e0[b]
+        if precision == "f32":
+            ci, ei = ci.astype(np.float32).astype(np.float64), ei.astype(np.float32).astype(np.float64)
+        rc, re_ = m.step_fs(ci, ei, steps)
+        assert rel_linf([gc[b], ge[b]], [rc, re_]) < tol, b
+
+
+@pytest.mark.parametrize("n", [(64, 32, 32), (16, 16, 32)])
+def test_batch_3d_fd_and_handoff(oracle, n):
+    # explicit FD on a 3D batch (one launch per replica and step; both 3D FD kernels: nx >= 64 marching, nx < 64 fused) and
+    # the FS -> FD -> FS hand-off
+    p, B = 2, 3
+    c, eta, dx = synth.init_b(n, p)
+    rng = np.random.default_rng(12)
+    c0 = np.stack([c + 0.02 * rng.standard_normal(c.shape) for _ in range(B)])
+    e0 = np.stack([eta + 0.01 * rng.standard_normal(eta.shape) for _ in range(B)])
+    with pf.Context(n, n_eta=p, dx=dx, dt=1e-3, nbatch=B) as ctx:
+        ctx.set_fields(c0, e0)
+        ctx.step_fs(4); ctx.step_fd(6); ctx.step_fs(3)
+        gc, ge = ctx.get_fields()
+    m = oracle.Model(n=n, n_eta=p, dx=dx, dt=1e-3)
+    for b in range(B):
+        rc, re_ = m.step_fs(c0[b], e0[b], 4)
+        rc, re_ = m.step_fd(rc, re_, 6)
+        rc, re_ = m.step_fs(rc, re_, 3)
+        assert rel_linf([gc[b], ge[b]], [rc, re_]) < 1e-10, b
