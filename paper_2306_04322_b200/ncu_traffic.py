@@ -81,11 +81,19 @@ def parse(csv_path: str):
                 per.setdefault(k, []).append(v)
         return per
     ki, ri, wi = head.index("Kernel Name"), head.index("dram__bytes_read.sum"), head.index("dram__bytes_write.sum")
+    gi = head.index("Grid Size") if "Grid Size" in head else None
     units = body[0]                                             # wide format: the second row holds the units
+    grids = {}
     for r in body[1:]:
         k = step_kernel_of(r[ki])
         if k:
-            per.setdefault(k, []).append(float(r[ri].replace(",", "")) * _UNIT[units[ri]] + float(r[wi].replace(",", "")) * _UNIT[units[wi]])
+            g = tuple(int(v) for v in re.findall(r"\d+", r[gi])) if gi is not None else ()
+            grids.setdefault(k, {}).setdefault(g, []).append(
+                float(r[ri].replace(",", "")) * _UNIT[units[ri]] + float(r[wi].replace(",", "")) * _UNIT[units[wi]])
+    # col2d_kernel also serves the one-off pass that fills the carried spectrum after pf_set_fields, with a smaller grid:
+    # a step launch is the one with the most CTAs
+    for k, by_grid in grids.items():
+        per[k] = by_grid[max(by_grid, key=lambda g: (g[0] * (g[1] if len(g) > 1 else 1) * (g[2] if len(g) > 2 else 1)) if g else 0)]
     return per
 
 
